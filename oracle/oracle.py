@@ -1,0 +1,123 @@
+"""ctypes loader for the CPU oracle (oracle/rk4ip_oracle.cpp).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+It builds liboracle.so with g++ on first use (no CUDA, no torch) and marshals numpy arrays; there is no
+arithmetic of the method in this file.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "rk4ip_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force=False):
+    """Compile oracle/rk4ip_oracle.cpp -> oracle/liboracle.so (plain g++, no fast-math)."""
+    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
+        return _LIB
+    tmp = _LIB + ".tmp.%d" % os.getpid()
+    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", tmp, _SRC]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        ll, i, d = ctypes.c_longlong, ctypes.c_int, ctypes.c_double
+        L.orc_dft.argtypes = [dp, dp, ll, i]
+        L.orc_fft.argtypes = [dp, ll, i]
+        L.orc_omega.argtypes = [dp, ll, d]
+        L.orc_linear_table.argtypes = [dp, i, ll, d, d, d, dp, i, i]
+        L.orc_apply_D.argtypes = [dp, i, ll, dp, i]
+        L.orc_nonlinear.argtypes = [dp, dp, i, ll, d, dp, i]
+        L.orc_rk4ip.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
+        for f in (L.orc_dft, L.orc_fft, L.orc_omega, L.orc_linear_table, L.orc_apply_D, L.orc_nonlinear,
+                  L.orc_rk4ip):
+            f.restype = i
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _c128(a):
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def default_threads():
+    return max(1, len(os.sched_getaffinity(0)))
+
+
+def dft(x, sign):
+    x = _c128(x)
+    out = np.empty_like(x)
+    assert lib().orc_dft(_p(x), _p(out), x.size, sign) == 0
+    return out
+
+
+def fft(x, sign):
+    x = _c128(x).copy()
+    assert lib().orc_fft(_p(x), x.size, sign) == 0
+    return x
+
+
+def omega(N, dt):
+    w = np.empty(N, dtype=np.float64)
+    assert lib().orc_omega(_p(w), N, dt) == 0
+    return w
+
+
+def linear_table(M, N, dt, hh, alpha, beta, nthreads=1):
+    beta = _f64(beta).reshape(M, -1)
+    E = np.empty((M, N), dtype=np.complex128)
+    assert lib().orc_linear_table(_p(E), M, N, dt, hh, alpha, _p(beta), beta.shape[1], nthreads) == 0
+    return E
+
+
+def apply_D(x, E, nthreads=1):
+    x = _c128(x).copy()
+    E = _c128(E)
+    M, N = E.shape
+    assert x.shape == (2 * M, N)
+    assert lib().orc_apply_D(_p(x), M, N, _p(E), nthreads) == 0
+    return x
+
+
+def nonlinear(u, hgamma, kappa, nthreads=1):
+    u = _c128(u)
+    R, N = u.shape
+    M = R // 2
+    kappa = _f64(kappa).reshape(M, M)
+    out = np.empty_like(u)
+    assert lib().orc_nonlinear(_p(u), _p(out), M, N, hgamma, _p(kappa), nthreads) == 0
+    return out
+
+
+def rk4ip(A, dt, h, alpha, beta, gamma, kappa, nsteps, nthreads=None):
+    """Return A advanced nsteps RK4IP steps.  A: (2M, N) complex128; beta: (M, K); kappa: (M, M)."""
+    A = _c128(A).copy()
+    R, N = A.shape
+    M = R // 2
+    assert R == 2 * M
+    beta = _f64(beta).reshape(M, -1)
+    kappa = _f64(kappa).reshape(M, M)
+    if nthreads is None:
+        nthreads = default_threads()
+    rc = lib().orc_rk4ip(_p(A), M, N, dt, h, alpha, _p(beta), beta.shape[1], gamma, _p(kappa), nsteps, nthreads)
+    assert rc == 0, "orc_rk4ip rejected its arguments"
+    return A

@@ -1,0 +1,293 @@
+// rk4ip_oracle.cpp — CPU ORACLE. TEST INFRASTRUCTURE ONLY.
+//
+// A plain, slow, obviously-correct fp64 implementation of the RK4IP step for the multimode
+// Manakov/NLSE, written from the paper (arXiv 1901.01895; citations are PAPER.md:<line>).
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// build, load or call this file.  It shares no code, header, table generator or helper with the
+// CUDA path under paper_1901_01895_b200/csrc/, and nothing in the product imports it.
+//
+// What is computed (every function cites the passage it follows):
+//   Eq. (1)  PAPER.md:35-37   dA_a/dz = L A_a + i*gamma*(sum_b kappa_ab |A_b|^2) A_a,
+//                             L = -alpha/2 + i*sum_n (i^n/n!) beta_{n,a} d^n/dt^n
+//   Eq. (6)  PAPER.md:75-88   the RK4IP step (6a)-(6f) with separation distance z' = z + h/2
+//   layout   PAPER.md:95,107  2M x N complex matrix, row-major, one row per spatial/polarisation mode
+//
+// Readings taken where the paper is silent or garbled:
+//   R1  Fourier sign: the time-domain operator of Eq. (1) is the authority.  With
+//       A(t) = sum_w At(w) exp(-i w t) one gets dAt/dz = (-alpha/2 + i sum_n beta_n w^n/n!) At,
+//       so "to frequency" is X_k = sum_n x_n exp(+2 pi i k n/N) and back carries exp(-...)/N.
+//   R2  sum_{n=0} runs over the K coefficients the caller supplies (n = 0..K-1).
+//   R3  Eq. (6b): k1 = exp(h/2 L)[ h N(A) A ]  (operator applied to the product).
+//   R4  Eq. (6e): k4 = h N(u4) u4 with u4 = exp(h/2 L)[A_I + k3].
+//   R5  |A_b|^2 of a Jones vector = |A_bx|^2 + |A_by|^2; rows 2a, 2a+1 are the x, y polarisations of mode a.
+//   R7  the Nyquist bin k = N/2 takes the negative frequency.
+//
+// Pins (tests/test_oracle_pins.py, -m "not gpu"): direct-DFT and library-FFT agreement, tone eigenvalue
+// exp(h L(W)), circular delay for beta_1, exact nonlinear phase rotation, energy decay exp(-alpha z),
+// soliton shape, 4th-order convergence against an independent adaptive integrator, integer exactness,
+// composition.  No function here is "parity unpinned".
+//
+// Numerical hygiene: twiddles and the dispersion phase are evaluated per index in long double
+// (never by recurrence); no -ffast-math.
+
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstring>
+#include <thread>
+#include <vector>
+
+namespace {
+
+typedef std::complex<double> cplx;
+const long double PI_L = 3.141592653589793238462643383279502884L;
+
+bool is_pow2(long long n) { return n >= 1 && (n & (n - 1)) == 0; }
+
+// run f(i) for i in [0, count) on up to nthreads std::threads (contiguous blocks; items are independent)
+template <class F>
+void parallel_for(long long count, int nthreads, F f) {
+  if (nthreads < 1) nthreads = 1;
+  if (nthreads == 1 || count < 2) {
+    for (long long i = 0; i < count; ++i) f(i);
+    return;
+  }
+  if ((long long)nthreads > count) nthreads = (int)count;
+  std::vector<std::thread> pool;
+  for (int w = 0; w < nthreads; ++w) {
+    long long lo = count * w / nthreads, hi = count * (w + 1) / nthreads;
+    pool.emplace_back([lo, hi, &f]() { for (long long i = lo; i < hi; ++i) f(i); });
+  }
+  for (auto& t : pool) t.join();
+}
+
+// exp(sign * 2 pi i p / N) for 0 <= p < N, in long double.  The angle is folded into the first octant with exact
+// integer arithmetic before sinl/cosl are called, so multiples of a quarter turn give exactly 0 and +-1 and the
+// table has the symmetries of the unit circle.
+void unit_root(long long p, long long N, int sign, long double* c, long double* s) {
+  long long q = 8 * p;            // position in eighths of a turn, scaled by N
+  int oct = (int)(q / N);         // octant 0..7
+  long long rem = q - (long long)oct * N;   // 0 <= rem < N, angle inside the octant = (rem/N) * (pi/4)
+  long double a;                  // folded angle in [0, pi/4]
+  if (oct & 1) a = (PI_L / 4.0L) * ((long double)(N - rem) / (long double)N);
+  else         a = (PI_L / 4.0L) * ((long double)rem / (long double)N);
+  long double ca = cosl(a), sa = sinl(a);
+  if (rem == 0 && !(oct & 1)) { ca = 1.0L; sa = 0.0L; }
+  long double cc, ss;
+  switch (oct) {
+    case 0: cc = ca;  ss = sa;  break;
+    case 1: cc = sa;  ss = ca;  break;
+    case 2: cc = -sa; ss = ca;  break;
+    case 3: cc = -ca; ss = sa;  break;
+    case 4: cc = -ca; ss = -sa; break;
+    case 5: cc = -sa; ss = -ca; break;
+    case 6: cc = sa;  ss = -ca; break;
+    default: cc = ca; ss = -sa; break;
+  }
+  *c = cc;
+  *s = (sign >= 0) ? ss : -ss;
+}
+
+// The plain definition of the discrete Fourier sum, O(N^2):  out_k = sum_n in_n exp(sign * 2 pi i k n / N).
+// (Definition of the DFT; sign = +1 is "to frequency" under reading R1.)
+void dft_direct(const cplx* in, cplx* out, long long N, int sign) {
+  for (long long k = 0; k < N; ++k) {
+    long double sr = 0.0L, si = 0.0L;
+    for (long long n = 0; n < N; ++n) {
+      long long p = (k * n) % N;  // exact integer phase index
+      long double c, s;
+      unit_root(p, N, sign, &c, &s);
+      sr += (long double)in[n].real() * c - (long double)in[n].imag() * s;
+      si += (long double)in[n].real() * s + (long double)in[n].imag() * c;
+    }
+    out[k] = cplx((double)sr, (double)si);
+  }
+}
+
+// Textbook iterative radix-2 decimation-in-time FFT (bit reversal, then log2 N butterfly stages),
+// unnormalised, same sum as dft_direct.  Twiddle j is exp(sign * 2 pi i j / N) from sinl/cosl.
+void fft_radix2(cplx* x, long long N, int sign) {
+  if (N < 2) return;
+  int lg = 0;
+  while ((1LL << lg) < N) ++lg;
+  for (long long i = 0; i < N; ++i) {
+    long long r = 0;
+    for (int b = 0; b < lg; ++b) if (i & (1LL << b)) r |= 1LL << (lg - 1 - b);
+    if (r > i) std::swap(x[i], x[r]);
+  }
+  std::vector<cplx> w(N / 2);
+  for (long long j = 0; j < N / 2; ++j) {
+    long double c, s;
+    unit_root(j, N, sign, &c, &s);
+    w[j] = cplx((double)c, (double)s);
+  }
+  for (long long len = 2; len <= N; len <<= 1) {
+    long long half = len / 2, step = N / len;
+    for (long long base = 0; base < N; base += len) {
+      for (long long j = 0; j < half; ++j) {
+        cplx t = w[j * step] * x[base + j + half];
+        cplx u = x[base + j];
+        x[base + j] = u + t;
+        x[base + j + half] = u - t;
+      }
+    }
+  }
+}
+
+// Angular frequency of bin k (reading R7): w_k = 2 pi k'/(N dt), k' = k for k < N/2, else k - N.
+long double omega_of_bin(long long k, long long N, double dt) {
+  long long ks = (k < N / 2) ? k : k - N;
+  return 2.0L * PI_L * (long double)ks / ((long double)N * (long double)dt);
+}
+
+// exp(hh * L_a(w_k)) with L_a(w) = -alpha/2 + i * sum_{n=0}^{K-1} beta_{n,a} w^n / n!   (Eq. 1; R1, R2)
+// hh is the distance the factor advances (h/2 inside a step).  Long double throughout, rounded once.
+cplx linear_factor(long double w, double hh, double alpha, const double* beta_a, int K) {
+  long double phase = 0.0L, wn = 1.0L, fact = 1.0L;
+  for (int n = 0; n < K; ++n) {
+    if (n > 0) { wn *= w; fact *= (long double)n; }
+    phase += (long double)beta_a[n] * wn / fact;
+  }
+  phase *= (long double)hh;
+  long double amp = expl(-(long double)alpha * (long double)hh / 2.0L);
+  return cplx((double)(amp * cosl(phase)), (double)(amp * sinl(phase)));
+}
+
+// E[a][k] for all modes and bins.
+void linear_table(cplx* E, int M, long long N, double dt, double hh, double alpha, const double* beta, int K,
+                  int nthreads) {
+  parallel_for((long long)M, nthreads, [&](long long a) {
+    for (long long k = 0; k < N; ++k)
+      E[a * N + k] = linear_factor(omega_of_bin(k, N, dt), hh, alpha, beta + a * K, K);
+  });
+}
+
+// D(x) = exp(hh L) x for every row: to frequency (sign +), multiply by E_a[k], back (sign -) and 1/N.
+// Row r belongs to mode a = r/2 (R5).  (Eq. 6a "exp(h/2 L) . A"; linear step per row)
+void apply_D(cplx* x, int M, long long N, const cplx* E, int nthreads) {
+  parallel_for(2LL * M, nthreads, [&](long long r) {
+    cplx* row = x + r * N;
+    const cplx* Ea = E + (r / 2) * N;
+    fft_radix2(row, N, +1);
+    for (long long k = 0; k < N; ++k) row[k] *= Ea[k];
+    fft_radix2(row, N, -1);
+    double inv = 1.0 / (double)N;
+    for (long long k = 0; k < N; ++k) row[k] *= inv;
+  });
+}
+
+// out_{a,p}[t] = (i * hgamma * S_a[t]) * u_{a,p}[t],  S_a[t] = sum_b kappa_ab P_b[t],  P_b = |u_bx|^2 + |u_by|^2
+// (Eq. 1 nonlinear part; h N(u) u of Eq. 6b-e with hgamma = h*gamma).  b ascending, plain loops.
+void nonlinear(const cplx* u, cplx* out, int M, long long N, double hgamma, const double* kappa, int nthreads) {
+  const long long BLK = 4096;
+  long long nblk = (N + BLK - 1) / BLK;
+  parallel_for(nblk, nthreads, [&](long long blk) {
+    std::vector<double> P(M);
+    long long t0 = blk * BLK, t1 = std::min(N, t0 + BLK);
+    for (long long t = t0; t < t1; ++t) {
+      for (int b = 0; b < M; ++b) {
+        cplx ux = u[(2LL * b) * N + t], uy = u[(2LL * b + 1) * N + t];
+        P[b] = (ux.real() * ux.real() + ux.imag() * ux.imag()) + (uy.real() * uy.real() + uy.imag() * uy.imag());
+      }
+      for (int a = 0; a < M; ++a) {
+        double S = 0.0;
+        for (int b = 0; b < M; ++b) S += kappa[(long long)a * M + b] * P[b];
+        double g = hgamma * S;
+        for (int p = 0; p < 2; ++p) {
+          cplx v = u[(2LL * a + p) * N + t];
+          out[(2LL * a + p) * N + t] = cplx(-g * v.imag(), g * v.real());  // (i g) * v
+        }
+      }
+    }
+  });
+}
+
+// One RK4IP step, Eq. (6a)-(6f) in the paper's order and notation (R3, R4).
+// E is the table for hh = h/2.  Seven full-size buffers, nothing fused or reordered.
+void rk4ip_step(cplx* A, int M, long long N, const cplx* E, double hgamma, const double* kappa, int nthreads,
+                cplx* AI, cplx* k1, cplx* k2, cplx* k3, cplx* k4, cplx* tmp) {
+  const long long tot = 2LL * M * N;
+  // (6a) A_I = exp(h/2 L) A
+  std::memcpy((void*)AI, (const void*)A, sizeof(cplx) * tot);
+  apply_D(AI, M, N, E, nthreads);
+  // (6b) k1 = exp(h/2 L) [ h N(A) A ]
+  nonlinear(A, k1, M, N, hgamma, kappa, nthreads);
+  apply_D(k1, M, N, E, nthreads);
+  // (6c) k2 = h N(A_I + k1/2) [A_I + k1/2]
+  for (long long i = 0; i < tot; ++i) tmp[i] = AI[i] + k1[i] / 2.0;
+  nonlinear(tmp, k2, M, N, hgamma, kappa, nthreads);
+  // (6d) k3 = h N(A_I + k2/2) [A_I + k2/2]
+  for (long long i = 0; i < tot; ++i) tmp[i] = AI[i] + k2[i] / 2.0;
+  nonlinear(tmp, k3, M, N, hgamma, kappa, nthreads);
+  // (6e) k4 = h N( exp(h/2 L)[A_I + k3] ) exp(h/2 L)[A_I + k3]
+  for (long long i = 0; i < tot; ++i) tmp[i] = AI[i] + k3[i];
+  apply_D(tmp, M, N, E, nthreads);
+  nonlinear(tmp, k4, M, N, hgamma, kappa, nthreads);
+  // (6f) A(z+h) = exp(h/2 L)[A_I + k1/6 + k2/3 + k3/3] + k4/6
+  for (long long i = 0; i < tot; ++i) tmp[i] = AI[i] + k1[i] / 6.0 + k2[i] / 3.0 + k3[i] / 3.0;
+  apply_D(tmp, M, N, E, nthreads);
+  for (long long i = 0; i < tot; ++i) A[i] = tmp[i] + k4[i] / 6.0;
+}
+
+}  // namespace
+
+extern "C" {
+
+// All complex arrays are interleaved (re, im) doubles.  Return 0 on success, -1 on bad arguments.
+
+int orc_dft(const double* in, double* out, long long N, int sign) {
+  if (!in || !out || N < 1 || (sign != 1 && sign != -1)) return -1;
+  dft_direct((const cplx*)in, (cplx*)out, N, sign);
+  return 0;
+}
+
+int orc_fft(double* x, long long N, int sign) {
+  if (!x || !is_pow2(N) || (sign != 1 && sign != -1)) return -1;
+  fft_radix2((cplx*)x, N, sign);
+  return 0;
+}
+
+int orc_omega(double* w, long long N, double dt) {
+  if (!w || N < 1 || !(dt > 0)) return -1;
+  for (long long k = 0; k < N; ++k) w[k] = (double)omega_of_bin(k, N, dt);
+  return 0;
+}
+
+// E[M][N] complex: exp(hh * L_a(w_k)); beta is [M][K] row-major, beta[a*K+n] = beta_{n,a}.
+int orc_linear_table(double* E, int M, long long N, double dt, double hh, double alpha, const double* beta, int K,
+                     int nthreads) {
+  if (!E || !beta || M < 1 || K < 1 || !is_pow2(N) || !(dt > 0)) return -1;
+  linear_table((cplx*)E, M, N, dt, hh, alpha, beta, K, nthreads);
+  return 0;
+}
+
+// x[2M][N] <- exp(hh L) x, E from orc_linear_table with the same hh.
+int orc_apply_D(double* x, int M, long long N, const double* E, int nthreads) {
+  if (!x || !E || M < 1 || !is_pow2(N)) return -1;
+  apply_D((cplx*)x, M, N, (const cplx*)E, nthreads);
+  return 0;
+}
+
+// out[2M][N] = (i * hgamma * sum_b kappa_ab P_b) * u;  kappa is [M][M] row-major, kappa[a*M+b] = kappa_ab.
+int orc_nonlinear(const double* u, double* out, int M, long long N, double hgamma, const double* kappa,
+                  int nthreads) {
+  if (!u || !out || !kappa || M < 1 || N < 1) return -1;
+  nonlinear((const cplx*)u, (cplx*)out, M, N, hgamma, kappa, nthreads);
+  return 0;
+}
+
+// A[2M][N] advanced nsteps RK4IP steps of size h, in place.
+int orc_rk4ip(double* A, int M, long long N, double dt, double h, double alpha, const double* beta, int K,
+              double gamma, const double* kappa, int nsteps, int nthreads) {
+  if (!A || !beta || !kappa || M < 1 || K < 1 || !is_pow2(N) || !(dt > 0) || nsteps < 0) return -1;
+  if (nsteps == 0) return 0;
+  const long long tot = 2LL * M * N;
+  std::vector<cplx> E((size_t)M * N), AI(tot), k1(tot), k2(tot), k3(tot), k4(tot), tmp(tot);
+  linear_table(E.data(), M, N, dt, h / 2.0, alpha, beta, K, nthreads);
+  for (int s = 0; s < nsteps; ++s)
+    rk4ip_step((cplx*)A, M, N, E.data(), h * gamma, kappa, nthreads, AI.data(), k1.data(), k2.data(), k3.data(),
+               k4.data(), tmp.data());
+  return 0;
+}
+
+}  // extern "C"
