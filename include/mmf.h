@@ -1,0 +1,97 @@
+/* mmf.h — C ABI of the B200-native RK4IP propagator for the multimode Manakov/NLSE.
+ *
+ * Source of truth for what is computed: arXiv 1901.01895 ("the paper"; citations are PAPER.md:<line> of the
+ * extracted text) — Eq. (1) PAPER.md:35-37 (model), Eq. (6a)-(6f) PAPER.md:75-88 (the RK4IP step), data layout
+ * PAPER.md:95,107 (2M x N complex matrix, row-major, one row per spatial/polarisation mode).  Readings taken where
+ * the paper is silent or garbled are listed in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - Units are the caller's: dt in [T], h in [L]; alpha in 1/[L] is the linear POWER attenuation (the amplitude
+ *     decays as exp(-alpha z/2), Eq. 1); beta_n in [T]^n/[L]; gamma in 1/(W [L]) with |A|^2 in W.
+ *   - Field layout: A[2M][N] complex128, interleaved (re, im), row-major; row r = 2a + p is polarisation p (0 = x,
+ *     1 = y) of spatial mode a.  |A_b|^2 of Eq. (1) is |A_bx|^2 + |A_by|^2 (Manakov).
+ *   - Fourier convention (Eq. 1 is written in the time domain; it fixes the convention): A(t) = sum_k At_k
+ *     exp(-i w_k t), w_k = 2 pi k'/(N dt), k' = k for k < N/2 and k - N otherwise (the Nyquist bin is negative);
+ *     then L_a(w) = -alpha/2 + i sum_{n=0}^{K-1} beta_{n,a} w^n / n!  and beta_1 > 0 DELAYS the field.
+ *   - Every function returns MMF_OK (0) or a negative error code; nothing throws, prints or keeps global state.
+ *     Plans are independent; one plan must not be used from two streams at once.
+ *   - "device" pointers are CUDA device pointers of the current device; "host" pointers are ordinary memory.
+ *   - Functions taking a stream only ENQUEUE work on it (no allocation, no synchronisation) unless stated.
+ */
+#ifndef MMF_H_
+#define MMF_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MMF_OK      0
+#define MMF_EINVAL -1   /* bad argument (null pointer, size, non-finite parameter, unset/small workspace, alignment) */
+#define MMF_ENOMEM -2   /* host or device allocation failed */
+#define MMF_ECUDA  -3   /* CUDA runtime / launch error */
+
+typedef struct mmf_plan mmf_plan; /* opaque */
+
+/* Create a plan for M spatial modes x 2 polarisations x N samples.
+ *   out    host, receives the plan.
+ *   M >= 1; N a power of two, 16 <= N <= 2^24; dt > 0 sample spacing; h step size (Eq. 6: separation z' = z+h/2).
+ *   alpha  power attenuation (Eq. 1, "-alpha/2").
+ *   beta   host, [M][K] row-major, beta[a*K + n] = beta_{n,a}, n = 0..K-1 (Eq. 1 Taylor coefficients), 1 <= K <= 8.
+ *   gamma  Kerr coefficient (Eq. 1).
+ *   kappa  host, [M][M] row-major, kappa[a*M + b] = kappa_ab (Eq. 1; need not be symmetric).
+ * beta and kappa are copied; the plan owns its small device tables (kappa, twiddles). */
+int mmf_plan_create(mmf_plan **out, int M, long long N, double dt, double h, double alpha, const double *beta, int K,
+                    double gamma, const double *kappa);
+
+/* Bytes of device workspace mmf_propagate needs: three full-field buffers (the RK4IP intermediates of Eq. 6) plus
+ * the tabulated exp(h/2 L_a(w_k)) of Eq. (6a) (one row per mode).  The caller allocates it (e.g. a torch uint8
+ * tensor), 256-byte aligned, and keeps it alive while the plan is used. */
+size_t mmf_plan_workspace_bytes(const mmf_plan *plan);
+
+/* Attach the workspace and fill the plan's tables in it (enqueues kernels on `cuda_stream`, a cudaStream_t passed
+ * as void*; 0 = default stream).  Must precede mmf_propagate / mmf_apply_*. */
+int mmf_plan_set_workspace(mmf_plan *plan, void *ws_dev, size_t bytes, void *cuda_stream);
+
+/* Advance A by nsteps RK4IP steps of size h, Eq. (6a)-(6f), in place.
+ *   A_dev  device, [2M][N] complex128 (layout above), 16-byte aligned.  nsteps >= 0 (0 is a no-op).
+ * Calling with n1 then n2 steps equals one call with n1+n2 steps. */
+int mmf_propagate(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
+
+/* Same, for a HOST field: copies A_host to an internal slot of the workspace-adjacent device buffer `A_dev_scratch`
+ * (device, [2M][N] complex128, caller-owned), propagates, copies back and SYNCHRONISES the stream.  A_host should be
+ * page-locked for full copy bandwidth.  This is the end-to-end entry point bench.py times. */
+int mmf_propagate_host(mmf_plan *plan, void *A_host, void *A_dev_scratch, int nsteps, void *cuda_stream);
+
+/* Stage-level entry points (each is a row group of the hot path; used by the parity tests).
+ * mmf_apply_linear:    X <- exp(h/2 L) X  (Eq. 6a: transform, multiply by exp(h/2 L_a(w_k)), transform back), in place.
+ * mmf_apply_nonlinear: OUT <- h N(U) U = i h gamma (sum_b kappa_ab |U_b|^2) U_a   (Eq. 1 / the bracket of Eq. 6b).
+ *                      U and OUT are device [2M][N] complex128 and may alias exactly (OUT == U) or not at all. */
+int mmf_apply_linear(mmf_plan *plan, void *X_dev, void *cuda_stream);
+int mmf_apply_nonlinear(mmf_plan *plan, const void *U_dev, void *OUT_dev, void *cuda_stream);
+
+/* Debug / test entry points.
+ * mmf_debug_forward:  SPEC <- the plain forward transform of every row of X, SPEC[r][k] = sum_n X[r][n] exp(+2 pi i k n/N),
+ *                     written in NATURAL bin order (the hot path never materialises this order).  X is destroyed.
+ * mmf_debug_freq_index: host int64 array idx[N]; idx[s] = the bin k that slot s of the plan's internal (permuted)
+ *                     spectrum layout holds.  Must be a permutation of 0..N-1.  Synchronises. */
+int mmf_debug_forward(mmf_plan *plan, void *X_dev, void *SPEC_dev, void *cuda_stream);
+int mmf_debug_freq_index(mmf_plan *plan, long long *idx_host);
+
+/* Number of kernel launches this plan has enqueued since creation (bench.py's gpu_launches). */
+long long mmf_plan_launch_count(const mmf_plan *plan);
+
+/* Frees the plan and its device tables (not the workspace, which the caller owns). */
+int mmf_plan_destroy(mmf_plan *plan);
+
+/* Static, human-readable text for a status code; for MMF_ECUDA the last CUDA error string seen by this thread. */
+const char *mmf_status_string(int status);
+
+/* Library version string. */
+const char *mmf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MMF_H_ */

@@ -1,0 +1,168 @@
+"""Thin Python binding of the C ABI in include/mmf.h (argument marshalling only — every step of the path runs in
+the CUDA kernels of libmmf_b200.so).  PyTorch is used for device buffers and streams, nothing else.
+
+There is no CPU fallback: if the CUDA library is missing or cannot be loaded, importing a symbol from here raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmmf_b200.so")
+
+MMF_OK, MMF_EINVAL, MMF_ENOMEM, MMF_ECUDA = 0, -1, -2, -3
+
+# every symbol include/mmf.h declares (tests check that the built library exports all of them)
+SYMBOLS = ["mmf_plan_create", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate",
+           "mmf_propagate_host", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
+           "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_destroy", "mmf_status_string", "mmf_version"]
+
+_lib = None
+
+
+class MmfError(RuntimeError):
+    pass
+
+
+def lib():
+    """Load libmmf_b200.so (built in-tree by paper_1901_01895_b200/build.py).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise MmfError("CUDA library %s is missing: run `python -m paper_1901_01895_b200.build` "
+                       "(there is no CPU fallback)" % LIB_PATH)
+    L = ctypes.CDLL(LIB_PATH)
+    vp, ll, i, d, sz = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    dp = ctypes.POINTER(ctypes.c_double)
+    L.mmf_plan_create.argtypes = [ctypes.POINTER(vp), i, ll, d, d, d, dp, i, d, dp]
+    L.mmf_plan_create.restype = i
+    L.mmf_plan_workspace_bytes.argtypes = [vp]
+    L.mmf_plan_workspace_bytes.restype = sz
+    L.mmf_plan_set_workspace.argtypes = [vp, vp, sz, vp]
+    L.mmf_plan_set_workspace.restype = i
+    L.mmf_propagate.argtypes = [vp, vp, i, vp]
+    L.mmf_propagate.restype = i
+    L.mmf_propagate_host.argtypes = [vp, vp, vp, i, vp]
+    L.mmf_propagate_host.restype = i
+    L.mmf_apply_linear.argtypes = [vp, vp, vp]
+    L.mmf_apply_linear.restype = i
+    L.mmf_apply_nonlinear.argtypes = [vp, vp, vp, vp]
+    L.mmf_apply_nonlinear.restype = i
+    L.mmf_debug_forward.argtypes = [vp, vp, vp, vp]
+    L.mmf_debug_forward.restype = i
+    L.mmf_debug_freq_index.argtypes = [vp, ctypes.POINTER(ll)]
+    L.mmf_debug_freq_index.restype = i
+    L.mmf_plan_launch_count.argtypes = [vp]
+    L.mmf_plan_launch_count.restype = ll
+    L.mmf_plan_destroy.argtypes = [vp]
+    L.mmf_plan_destroy.restype = i
+    L.mmf_status_string.argtypes = [i]
+    L.mmf_status_string.restype = ctypes.c_char_p
+    L.mmf_version.argtypes = []
+    L.mmf_version.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc, what):
+    if rc != MMF_OK:
+        raise MmfError("%s failed: %s (%d)" % (what, lib().mmf_status_string(rc).decode(), rc))
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+class Plan:
+    """mmf_plan_create / mmf_plan_set_workspace / mmf_propagate / mmf_plan_destroy with torch-owned buffers."""
+
+    def __init__(self, M, N, dt, h, alpha, beta, gamma, kappa, device="cuda:0"):
+        import torch
+        L = lib()
+        self.M, self.N = int(M), int(N)
+        beta = np.ascontiguousarray(beta, dtype=np.float64).reshape(self.M, -1)
+        kappa = np.ascontiguousarray(kappa, dtype=np.float64).reshape(self.M, self.M)
+        self._h = ctypes.c_void_p()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        dp = ctypes.POINTER(ctypes.c_double)
+        rc = L.mmf_plan_create(ctypes.byref(self._h), self.M, self.N, float(dt), float(h), float(alpha),
+                               beta.ctypes.data_as(dp), beta.shape[1], float(gamma), kappa.ctypes.data_as(dp))
+        _check(rc, "mmf_plan_create")
+        nbytes = L.mmf_plan_workspace_bytes(self._h)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-self.workspace.data_ptr()) % 256
+        self._ws_ptr = self.workspace.data_ptr() + off
+        _check(L.mmf_plan_set_workspace(self._h, ctypes.c_void_p(self._ws_ptr), nbytes, _stream_ptr()),
+               "mmf_plan_set_workspace")
+
+    # -- helpers -------------------------------------------------------------------------------------------
+    def _field_ptr(self, A):
+        import torch
+        assert A.is_cuda and A.dtype == torch.complex128 and A.is_contiguous()
+        assert tuple(A.shape) == (2 * self.M, self.N), (A.shape, self.M, self.N)
+        return ctypes.c_void_p(A.data_ptr())
+
+    # -- the C ABI -------------------------------------------------------------------------------------------
+    def propagate(self, A, nsteps, stream=None):
+        """A: torch complex128 CUDA tensor (2M, N), advanced in place by nsteps RK4IP steps."""
+        _check(lib().mmf_propagate(self._h, self._field_ptr(A), int(nsteps), _stream_ptr(stream)), "mmf_propagate")
+        return A
+
+    def propagate_host(self, A_host, A_scratch, nsteps, stream=None):
+        """A_host: pinned torch complex128 CPU tensor (2M, N); A_scratch: CUDA tensor of the same shape."""
+        import torch
+        assert (not A_host.is_cuda) and A_host.dtype == torch.complex128 and A_host.is_contiguous()
+        assert tuple(A_host.shape) == (2 * self.M, self.N)
+        _check(lib().mmf_propagate_host(self._h, ctypes.c_void_p(A_host.data_ptr()), self._field_ptr(A_scratch),
+                                        int(nsteps), _stream_ptr(stream)), "mmf_propagate_host")
+        return A_host
+
+    def apply_linear(self, X, stream=None):
+        _check(lib().mmf_apply_linear(self._h, self._field_ptr(X), _stream_ptr(stream)), "mmf_apply_linear")
+        return X
+
+    def apply_nonlinear(self, U, OUT, stream=None):
+        _check(lib().mmf_apply_nonlinear(self._h, self._field_ptr(U), self._field_ptr(OUT), _stream_ptr(stream)),
+               "mmf_apply_nonlinear")
+        return OUT
+
+    def debug_forward(self, X, SPEC, stream=None):
+        _check(lib().mmf_debug_forward(self._h, self._field_ptr(X), self._field_ptr(SPEC), _stream_ptr(stream)),
+               "mmf_debug_forward")
+        return SPEC
+
+    def debug_freq_index(self):
+        idx = np.empty(self.N, dtype=np.int64)
+        _check(lib().mmf_debug_freq_index(self._h, idx.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong))),
+               "mmf_debug_freq_index")
+        return idx
+
+    def launch_count(self):
+        return int(lib().mmf_plan_launch_count(self._h))
+
+    def destroy(self):
+        if self._h:
+            lib().mmf_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def raw_create(M, N, dt, h, alpha, beta, K, gamma, kappa):
+    """mmf_plan_create with raw arguments (for error-path tests).  Returns (status, handle)."""
+    h_ = ctypes.c_void_p()
+    dp = ctypes.POINTER(ctypes.c_double)
+    b = None if beta is None else np.ascontiguousarray(beta, dtype=np.float64).ctypes.data_as(dp)
+    k = None if kappa is None else np.ascontiguousarray(kappa, dtype=np.float64).ctypes.data_as(dp)
+    rc = lib().mmf_plan_create(ctypes.byref(h_), int(M), int(N), float(dt), float(h), float(alpha), b, int(K),
+                               float(gamma), k)
+    return rc, h_

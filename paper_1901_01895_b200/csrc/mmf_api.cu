@@ -1,0 +1,411 @@
+// mmf_api.cu — the C ABI of include/mmf.h: plan management, table generation and the per-step launch sequence.
+// The product path: every step of the hot path runs in the kernels of kernels.cuh; there is no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/mmf.h"
+#include "kernels.cuh"
+
+using namespace mmf;
+
+namespace {
+
+thread_local char g_cuda_msg[256] = "CUDA error";
+
+int cuda_fail(cudaError_t e) {
+  snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: %s", cudaGetErrorString(e));
+  return MMF_ECUDA;
+}
+#define CU(call)                                \
+  do {                                          \
+    cudaError_t e__ = (call);                   \
+    if (e__ != cudaSuccess) return cuda_fail(e__); \
+  } while (0)
+
+constexpr int cols_logw(int logn1) { return logn1 <= 8 ? 4 : logn1 == 9 ? 3 : logn1 <= 11 ? 2 : 1; }
+constexpr int rows_logb(int logn2) { return logn2 >= 9 ? 0 : 9 - logn2; }
+
+// exp(2 pi i p / n) for 0 <= p < n (n a power of two), long double with the angle folded to [0, pi/4] first,
+// so that the table is exactly symmetric and quarter turns are exact.  (Written independently of the oracle.)
+void root_of_unity(long long p, long long n, double* re, double* im) {
+  static const long double TWO_PI = 6.283185307179586476925286766559005768L;
+  p %= n;
+  const long long quarter = n / 4;
+  long double c, s;
+  if (n < 8) {  // n = 1, 2, 4: all values exact
+    static const int C4[4] = {1, 0, -1, 0}, S4[4] = {0, 1, 0, -1};
+    const int q = (int)(p * (4 / n));
+    *re = C4[q];
+    *im = S4[q];
+    return;
+  }
+  const int quad = (int)(p / quarter);
+  long long r = p % quarter;  // angle r/n turns inside the quadrant, 0 <= r < n/4
+  bool swap = false;
+  if (r > quarter / 2) {  // fold about the diagonal of the quadrant
+    r = quarter - r;
+    swap = true;
+  }
+  if (r == 0) {
+    c = 1.0L;
+    s = 0.0L;
+  } else if (2 * r == quarter && !swap) {
+    c = s = 0.707106781186547524400844362104849039L;
+  } else {
+    const long double ang = TWO_PI * (long double)r / (long double)n;
+    c = cosl(ang);
+    s = sinl(ang);
+  }
+  if (swap) {
+    const long double tmp = c;
+    c = s;
+    s = tmp;
+  }
+  long double cr, ci;
+  switch (quad) {
+    case 0: cr = c; ci = s; break;
+    case 1: cr = -s; ci = c; break;
+    case 2: cr = -c; ci = -s; break;
+    default: cr = s; ci = -c; break;
+  }
+  *re = (double)cr;
+  *im = (double)ci;
+}
+
+int upload_roots(cpx** dptr, long long count, long long step, long long n) {
+  std::vector<cpx> h((size_t)count);
+  for (long long i = 0; i < count; ++i) root_of_unity(i * step, n, &h[i].x, &h[i].y);
+  CU(cudaMalloc((void**)dptr, sizeof(cpx) * (size_t)count));
+  CU(cudaMemcpy(*dptr, h.data(), sizeof(cpx) * (size_t)count, cudaMemcpyHostToDevice));
+  return MMF_OK;
+}
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+struct mmf_plan {
+  int M = 0, K = 0, logn = 0, logn1 = 0, logn2 = 0, lb = 0;
+  long long N = 0;
+  double dt = 0, h = 0, alpha = 0, gamma = 0;
+  std::vector<double> beta, kappa;
+  double* d_kappa = nullptr;
+  cpx *d_tw1 = nullptr, *d_tw2 = nullptr, *d_whi = nullptr, *d_wlo = nullptr;
+  dd* d_coefs = nullptr;
+  unsigned char* ws = nullptr;
+  size_t ws_bytes = 0, field_bytes = 0;
+  cpx *Y = nullptr, *Z = nullptr, *W = nullptr, *E = nullptr;
+  long long launches = 0;
+};
+
+namespace {
+
+// ---- launch helpers ----------------------------------------------------------------------------------------------
+template <int LOGN1, int DIR>
+int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
+  constexpr int LOGW = cols_logw(LOGN1);
+  constexpr int LOGTOT = LOGN1 + LOGW;
+  constexpr size_t smem = sizeof(cpx) << LOGTOT;
+  auto kern = k_cols<LOGN1, LOGW, DIR>;
+  static bool attr_done = false;
+  if (!attr_done) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_done = true;
+  }
+  dim3 grid((unsigned)(1u << (p->logn2 - LOGW)), (unsigned)(2 * p->M), (unsigned)nbuf);
+  TwoLevelTw tw{p->d_whi, p->d_wlo, p->lb};
+  kern<<<grid, 1 << (LOGTOT - 4), smem, st>>>(X0, X1, p->d_tw1, tw, p->logn2);
+  p->launches++;
+  CU(cudaGetLastError());
+  return MMF_OK;
+}
+
+template <int DIR>
+int launch_cols(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
+  switch (p->logn1) {
+    case 6: return launch_cols_t<6, DIR>(p, X0, X1, nbuf, st);
+    case 7: return launch_cols_t<7, DIR>(p, X0, X1, nbuf, st);
+    case 8: return launch_cols_t<8, DIR>(p, X0, X1, nbuf, st);
+    case 9: return launch_cols_t<9, DIR>(p, X0, X1, nbuf, st);
+    case 10: return launch_cols_t<10, DIR>(p, X0, X1, nbuf, st);
+    case 11: return launch_cols_t<11, DIR>(p, X0, X1, nbuf, st);
+    case 12: return launch_cols_t<12, DIR>(p, X0, X1, nbuf, st);
+    default: return MMF_EINVAL;
+  }
+}
+
+template <int LOGN2, int MODE>
+int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
+  constexpr int LOGB = rows_logb(LOGN2);
+  constexpr int LOGTOT = LOGN2 + LOGB;
+  constexpr size_t smem = sizeof(cpx) << LOGTOT;
+  auto kern = k_rows<LOGN2, LOGB, MODE>;
+  static bool attr_done = false;
+  if (!attr_done) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_done = true;
+  }
+  const long long nchunks = (2LL * p->M) << p->logn1;
+  dim3 grid((unsigned)((nchunks + (1 << LOGB) - 1) >> LOGB), 1, (unsigned)nbuf);
+  kern<<<grid, 1 << (LOGTOT - 4), smem, st>>>(X0, X1, p->E, p->d_tw2, nchunks, p->logn1);
+  p->launches++;
+  CU(cudaGetLastError());
+  return MMF_OK;
+}
+
+template <int MODE>
+int launch_rows(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
+  switch (p->logn2) {
+    case 4: return launch_rows_t<4, MODE>(p, X0, X1, nbuf, st);
+    case 5: return launch_rows_t<5, MODE>(p, X0, X1, nbuf, st);
+    case 6: return launch_rows_t<6, MODE>(p, X0, X1, nbuf, st);
+    case 7: return launch_rows_t<7, MODE>(p, X0, X1, nbuf, st);
+    case 8: return launch_rows_t<8, MODE>(p, X0, X1, nbuf, st);
+    case 9: return launch_rows_t<9, MODE>(p, X0, X1, nbuf, st);
+    case 10: return launch_rows_t<10, MODE>(p, X0, X1, nbuf, st);
+    case 11: return launch_rows_t<11, MODE>(p, X0, X1, nbuf, st);
+    case 12: return launch_rows_t<12, MODE>(p, X0, X1, nbuf, st);
+    default: return MMF_EINVAL;
+  }
+}
+
+// D on one or two full-field buffers: exp(h/2 L) in place (rows a1-a3 of the hot path).
+int apply_D(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
+  int rc;
+  if (p->logn1 > 0 && (rc = launch_cols<0>(p, X0, X1, nbuf, st)) != MMF_OK) return rc;
+  if ((rc = launch_rows<0>(p, X0, X1, nbuf, st)) != MMF_OK) return rc;
+  if (p->logn1 > 0 && (rc = launch_cols<1>(p, X0, X1, nbuf, st)) != MMF_OK) return rc;
+  return MMF_OK;
+}
+
+size_t nl_smem_bytes(const mmf_plan* p) { return sizeof(double) * 2 * (size_t)p->M * MMF_NL_T; }
+
+template <int MODE>
+int launch_nl(mmf_plan* p, cpx* X, cpx* Y, cpx* Z, cpx* W, cudaStream_t st) {
+  auto kern = k_nl<MODE>;
+  const size_t smem = nl_smem_bytes(p);
+  static size_t attr_smem = 0;
+  if (smem > attr_smem) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_smem = smem;
+  }
+  NlParams q;
+  q.X = X; q.Y = Y; q.Z = Z; q.W = W;
+  q.kappa = p->d_kappa;
+  q.hg = p->h * p->gamma;
+  q.M = p->M;
+  q.N = p->N;
+  const unsigned grid = (unsigned)((p->N + MMF_NL_T - 1) / MMF_NL_T);
+  kern<<<grid, MMF_NL_T * MMF_NL_WARPS, smem, st>>>(q);
+  p->launches++;
+  CU(cudaGetLastError());
+  return MMF_OK;
+}
+
+bool finite_all(const double* v, size_t n) {
+  for (size_t i = 0; i < n; ++i)
+    if (!std::isfinite(v[i])) return false;
+  return true;
+}
+
+void free_tables(mmf_plan* p) {
+  cudaFree(p->d_kappa);
+  cudaFree(p->d_tw1);
+  cudaFree(p->d_tw2);
+  cudaFree(p->d_whi);
+  cudaFree(p->d_wlo);
+  cudaFree(p->d_coefs);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mmf_version(void) { return "mmf-b200 0.1"; }
+
+const char* mmf_status_string(int status) {
+  switch (status) {
+    case MMF_OK: return "ok";
+    case MMF_EINVAL: return "invalid argument";
+    case MMF_ENOMEM: return "out of memory";
+    case MMF_ECUDA: return g_cuda_msg;
+    default: return "unknown status";
+  }
+}
+
+int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, double alpha, const double* beta, int K,
+                    double gamma, const double* kappa) {
+  if (!out) return MMF_EINVAL;
+  *out = nullptr;
+  if (!beta || !kappa || M < 1 || K < 1 || K > MMF_MAXK) return MMF_EINVAL;
+  if (N < 16 || N > (1LL << 24) || (N & (N - 1)) != 0) return MMF_EINVAL;
+  if (!(dt > 0) || !std::isfinite(dt) || !std::isfinite(h) || !std::isfinite(alpha) || !std::isfinite(gamma))
+    return MMF_EINVAL;
+  if (!finite_all(beta, (size_t)M * K) || !finite_all(kappa, (size_t)M * M)) return MMF_EINVAL;
+  if (sizeof(double) * 2 * (size_t)M * MMF_NL_T > 227 * 1024) return MMF_EINVAL;  // mode-power tile must fit one SM
+  mmf_plan* p = new (std::nothrow) mmf_plan;
+  if (!p) return MMF_ENOMEM;
+  p->M = M; p->K = K; p->N = N; p->dt = dt; p->h = h; p->alpha = alpha; p->gamma = gamma;
+  p->beta.assign(beta, beta + (size_t)M * K);
+  p->kappa.assign(kappa, kappa + (size_t)M * M);
+  int logn = 0;
+  while ((1LL << logn) < N) ++logn;
+  p->logn = logn;
+  if (logn <= 12) {
+    p->logn1 = 0;
+    p->logn2 = logn;
+  } else {
+    p->logn2 = (logn + 1) / 2;
+    p->logn1 = logn - p->logn2;
+  }
+  p->lb = (logn + 1) / 2;
+  p->field_bytes = sizeof(cpx) * 2 * (size_t)M * (size_t)N;
+  int rc = MMF_OK;
+  do {
+    cudaError_t e = cudaMalloc((void**)&p->d_kappa, sizeof(double) * (size_t)M * M);
+    if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MMF_ENOMEM : cuda_fail(e); break; }
+    e = cudaMemcpy(p->d_kappa, kappa, sizeof(double) * (size_t)M * M, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+    if ((rc = upload_roots(&p->d_tw2, 1LL << p->logn2, 1, 1LL << p->logn2)) != MMF_OK) break;
+    if (p->logn1 > 0) {
+      if ((rc = upload_roots(&p->d_tw1, 1LL << p->logn1, 1, 1LL << p->logn1)) != MMF_OK) break;
+      if ((rc = upload_roots(&p->d_wlo, 1LL << p->lb, 1, N)) != MMF_OK) break;
+      if ((rc = upload_roots(&p->d_whi, 1LL << (logn - p->lb), 1LL << p->lb, N)) != MMF_OK) break;
+    }
+    // per-mode phase coefficients hh * beta_n / n! in double-double (hh = h/2, Eq. 6a)
+    std::vector<dd> coefs((size_t)M * K);
+    for (int a = 0; a < M; ++a) {
+      double fact = 1.0;
+      for (int n = 0; n < K; ++n) {
+        if (n > 0) fact *= n;
+        coefs[(size_t)a * K + n] = dd_div_d(dd_two_prod(0.5 * h, beta[(size_t)a * K + n]), fact);
+      }
+    }
+    e = cudaMalloc((void**)&p->d_coefs, sizeof(dd) * coefs.size());
+    if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+    e = cudaMemcpy(p->d_coefs, coefs.data(), sizeof(dd) * coefs.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+  } while (0);
+  if (rc != MMF_OK) {
+    free_tables(p);
+    delete p;
+    return rc;
+  }
+  *out = p;
+  return MMF_OK;
+}
+
+size_t mmf_plan_workspace_bytes(const mmf_plan* p) {
+  if (!p) return 0;
+  const size_t F = align_up(p->field_bytes, 256);
+  const size_t E = align_up(sizeof(cpx) * (size_t)p->M * (size_t)p->N, 256);
+  return 3 * F + E;
+}
+
+int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_stream) {
+  if (!p || !ws_dev) return MMF_EINVAL;
+  if (bytes < mmf_plan_workspace_bytes(p) || ((size_t)ws_dev & 255) != 0) return MMF_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t F = align_up(p->field_bytes, 256);
+  p->ws = (unsigned char*)ws_dev;
+  p->ws_bytes = bytes;
+  p->Y = (cpx*)(p->ws);
+  p->Z = (cpx*)(p->ws + F);
+  p->W = (cpx*)(p->ws + 2 * F);
+  p->E = (cpx*)(p->ws + 3 * F);
+  EtabParams P;
+  memset(&P, 0, sizeof(P));
+  static const dd TWO_PI_DD = {6.283185307179586232e+00, 2.449293598294706414e-16};
+  P.twopi = TWO_PI_DD;
+  P.wstep = dd_div_d(TWO_PI_DD, (double)p->N * p->dt);
+  P.amp = std::exp(-p->alpha * p->h / 4.0) / (double)p->N;
+  P.K = p->K;
+  P.logn1 = p->logn1;
+  P.logn2 = p->logn2;
+  dim3 grid((unsigned)((p->N + 255) / 256), (unsigned)p->M);
+  k_etab<<<grid, 256, 0, st>>>(p->E, p->d_coefs, P);
+  p->launches++;
+  CU(cudaGetLastError());
+  return MMF_OK;
+}
+
+int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
+  if (!p || !A_dev || nsteps < 0 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
+  if (!p->ws) return MMF_EINVAL;
+  if (nsteps == 0) return MMF_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cpx *X = (cpx*)A_dev, *Y = p->Y, *Z = p->Z, *W = p->W;
+  int rc;
+  // the bracket of Eq. (6b) for the first step; later steps get it from NL_FINAL_NEXT
+  if ((rc = launch_nl<NL_PLAIN>(p, X, Y, Z, W, st)) != MMF_OK) return rc;
+  for (int s = 0; s < nsteps; ++s) {
+    if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;               // (6a) A_I, (6b) k1
+    if ((rc = launch_nl<NL_STAGE2>(p, X, Y, Z, W, st)) != MMF_OK) return rc;  // (6c) k2
+    if ((rc = launch_nl<NL_STAGE3>(p, X, Y, Z, W, st)) != MMF_OK) return rc;  // (6d) k3 and both brackets
+    if ((rc = apply_D(p, W, Z, 2, st)) != MMF_OK) return rc;               // (6e) argument, (6f) first term
+    if (s + 1 < nsteps) rc = launch_nl<NL_FINAL_NEXT>(p, X, Y, Z, W, st);  // (6e)+(6f), and next (6b) bracket
+    else rc = launch_nl<NL_FINAL>(p, X, Y, Z, W, st);
+    if (rc != MMF_OK) return rc;
+  }
+  return MMF_OK;
+}
+
+int mmf_propagate_host(mmf_plan* p, void* A_host, void* A_dev_scratch, int nsteps, void* cuda_stream) {
+  if (!p || !A_host || !A_dev_scratch || nsteps < 0) return MMF_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CU(cudaMemcpyAsync(A_dev_scratch, A_host, p->field_bytes, cudaMemcpyHostToDevice, st));
+  int rc = mmf_propagate(p, A_dev_scratch, nsteps, cuda_stream);
+  if (rc != MMF_OK) return rc;
+  CU(cudaMemcpyAsync(A_host, A_dev_scratch, p->field_bytes, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  return MMF_OK;
+}
+
+int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
+  if (!p || !X_dev || !p->ws || ((size_t)X_dev & 15) != 0) return MMF_EINVAL;
+  return apply_D(p, (cpx*)X_dev, (cpx*)X_dev, 1, (cudaStream_t)cuda_stream);
+}
+
+int mmf_apply_nonlinear(mmf_plan* p, const void* U_dev, void* OUT_dev, void* cuda_stream) {
+  if (!p || !U_dev || !OUT_dev || (((size_t)U_dev | (size_t)OUT_dev) & 15) != 0) return MMF_EINVAL;
+  return launch_nl<NL_PLAIN>(p, (cpx*)U_dev, (cpx*)OUT_dev, nullptr, nullptr, (cudaStream_t)cuda_stream);
+}
+
+int mmf_debug_forward(mmf_plan* p, void* X_dev, void* SPEC_dev, void* cuda_stream) {
+  if (!p || !X_dev || !SPEC_dev || X_dev == SPEC_dev) return MMF_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc;
+  if (p->logn1 > 0 && (rc = launch_cols<0>(p, (cpx*)X_dev, (cpx*)X_dev, 1, st)) != MMF_OK) return rc;
+  if ((rc = launch_rows<1>(p, (cpx*)X_dev, (cpx*)X_dev, 1, st)) != MMF_OK) return rc;
+  dim3 grid((unsigned)((p->N + 255) / 256), (unsigned)(2 * p->M));
+  k_unpermute<<<grid, 256, 0, st>>>((const cpx*)X_dev, (cpx*)SPEC_dev, p->logn1, p->logn2);
+  p->launches++;
+  CU(cudaGetLastError());
+  return MMF_OK;
+}
+
+int mmf_debug_freq_index(mmf_plan* p, long long* idx_host) {
+  if (!p || !idx_host) return MMF_EINVAL;
+  long long* d = nullptr;
+  CU(cudaMalloc((void**)&d, sizeof(long long) * (size_t)p->N));
+  k_slot_map<<<(unsigned)((p->N + 255) / 256), 256>>>(d, p->logn1, p->logn2);
+  p->launches++;
+  cudaError_t e = cudaMemcpy(idx_host, d, sizeof(long long) * (size_t)p->N, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return cuda_fail(e);
+  return MMF_OK;
+}
+
+long long mmf_plan_launch_count(const mmf_plan* p) { return p ? p->launches : 0; }
+
+int mmf_plan_destroy(mmf_plan* p) {
+  if (!p) return MMF_EINVAL;
+  free_tables(p);
+  delete p;
+  return MMF_OK;
+}
+
+}  // extern "C"

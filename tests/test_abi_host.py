@@ -1,0 +1,52 @@
+"""Host-side checks of the C ABI (no GPU): the library loads, exports every symbol include/mmf.h declares, and the
+argument validation that precedes any CUDA call returns MMF_EINVAL."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def mmf():
+    from paper_1901_01895_b200 import build, binding
+    build.build()
+    return binding
+
+
+def test_library_exports_every_declared_symbol(mmf):
+    hdr = open(os.path.join(ROOT, "include", "mmf.h")).read()
+    declared = set(re.findall(r"\b(mmf_[a-z_]+)\s*\(", hdr))
+    assert declared == set(mmf.SYMBOLS), declared ^ set(mmf.SYMBOLS)
+    L = mmf.lib()
+    for s in declared:
+        assert hasattr(L, s), s
+    assert L.mmf_version().startswith(b"mmf-b200")
+    assert L.mmf_status_string(mmf.MMF_EINVAL) == b"invalid argument"
+
+
+def test_create_rejects_bad_arguments_before_touching_cuda(mmf):
+    ok = dict(M=2, N=4096, dt=1.0, h=100.0, alpha=0.0, beta=np.zeros((2, 4)), K=4, gamma=1e-3, kappa=np.eye(2))
+    bad = [dict(N=4000), dict(N=8), dict(N=1 << 25), dict(M=0), dict(K=0), dict(K=9), dict(dt=0.0), dict(dt=-1.0),
+           dict(h=float("nan")), dict(gamma=float("inf")), dict(beta=None), dict(kappa=None),
+           dict(kappa=np.array([[1.0, np.nan], [0.0, 1.0]]))]
+    for b in bad:
+        kw = dict(ok)
+        kw.update(b)
+        rc, h = mmf.raw_create(kw["M"], kw["N"], kw["dt"], kw["h"], kw["alpha"], kw["beta"], kw["K"], kw["gamma"],
+                               kw["kappa"])
+        assert rc == mmf.MMF_EINVAL and not h.value, b
+    L = mmf.lib()
+    assert L.mmf_plan_workspace_bytes(None) == 0
+    assert L.mmf_plan_destroy(None) == mmf.MMF_EINVAL
+    assert L.mmf_propagate(None, None, 1, None) == mmf.MMF_EINVAL
+    assert L.mmf_plan_launch_count(None) == 0
+
+
+def test_missing_library_fails_loudly(mmf, monkeypatch):
+    monkeypatch.setattr(mmf, "_lib", None)
+    monkeypatch.setattr(mmf, "LIB_PATH", "/nonexistent/libmmf_b200.so")
+    with pytest.raises(mmf.MmfError):
+        mmf.lib()

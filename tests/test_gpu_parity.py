@@ -1,0 +1,220 @@
+"""GPU parity tests: the CUDA path (through the C ABI of include/mmf.h) against the CPU oracle, element by element on
+the same seeded inputs.  Bars: bit-exact for integer / index work; relative L2 <= 1e-10 per field for propagated
+fields (BASELINE.json north_star); tighter, arithmetic-derived bounds for single operators.
+"""
+import numpy as np
+import pytest
+
+from paper_1901_01895_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD = 1e-10          # north_star: relative L2 per field after the stated number of steps
+TOL_OP = 2e-14             # one transform pair / one operator: ~ log2(N) * eps, generous
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def mmf():
+    from paper_1901_01895_b200 import binding
+    binding.lib()           # fail loudly if the CUDA library is missing
+    return binding
+
+
+def to_dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+
+
+def plan_for(mmf, p, **over):
+    kw = dict(M=p.M, N=p.N, dt=p.dt, h=p.h, alpha=p.alpha, beta=p.beta, gamma=p.gamma, kappa=p.kappa)
+    kw.update(over)
+    return mmf.Plan(**kw)
+
+
+def rand_c(rng, *shape):
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+# ------------------------------------------------------------------------------------------ index permutation (P10 i)
+@pytest.mark.parametrize("logn", [4, 5, 9, 12, 13, 16, 18, 22])
+def test_slot_map_is_a_permutation(mmf, torch, logn):
+    N = 1 << logn
+    pl = mmf.Plan(1, N, 1.0, 1.0, 0.0, np.zeros((1, 1)), 0.0, np.ones((1, 1)))
+    idx = pl.debug_freq_index()
+    assert idx.min() == 0 and idx.max() == N - 1
+    assert np.array_equal(np.sort(idx), np.arange(N))
+
+
+# ----------------------------------------------------------------------------------------------- forward transform
+@pytest.mark.parametrize("logn", [4, 6, 7, 11, 12, 13, 14, 16])
+def test_forward_transform_matches_oracle(mmf, torch, orc, logn):
+    N, M = 1 << logn, 2
+    rng = np.random.default_rng(logn)
+    x = rand_c(rng, 2 * M, N)
+    pl = mmf.Plan(M, N, 1.0, 1.0, 0.0, np.zeros((M, 1)), 0.0, np.eye(M))
+    X = to_dev(torch, x)
+    S = torch.empty_like(X)
+    pl.debug_forward(X, S)
+    got = S.cpu().numpy()
+    for r in range(2 * M):
+        want = orc.fft(x[r], +1)
+        assert workloads.rel_l2_per_field(got[r], want) <= TOL_OP
+
+
+@pytest.mark.parametrize("logn", [4, 8, 12, 14])
+def test_forward_transform_integer_exact(mmf, torch, orc, logn):
+    """Gaussian integers on every (N/4)-th sample: only the twiddles 1, i, -1, -i meet non-zero data, all sums are
+    exact in fp64, so CUDA and oracle must agree BIT FOR BIT (P10 iii)."""
+    N, M = 1 << logn, 1
+    rng = np.random.default_rng(100 + logn)
+    x = np.zeros((2, N), dtype=complex)
+    x[:, :: N // 4] = rng.integers(-1000, 1000, size=(2, 4)) + 1j * rng.integers(-1000, 1000, size=(2, 4))
+    pl = mmf.Plan(M, N, 1.0, 1.0, 0.0, np.zeros((M, 1)), 0.0, np.eye(M))
+    X = to_dev(torch, x)
+    S = torch.empty_like(X)
+    pl.debug_forward(X, S)
+    got = S.cpu().numpy()
+    for r in range(2):
+        assert np.array_equal(got[r], orc.fft(x[r], +1))
+
+
+# ------------------------------------------------------------------------------------------------ linear operator D
+@pytest.mark.parametrize("cfg,M,logn", [(0, 2, 12), (1, 3, 13), (1, 2, 16), (2, 3, 14), (3, 5, 18), (4, 2, 15), (4, 1, 4)])
+def test_linear_operator_matches_oracle(mmf, torch, orc, cfg, M, logn):
+    p = workloads.problem(cfg, M=M, N=1 << logn)
+    A = p.field()
+    pl = plan_for(mmf, p)
+    X = to_dev(torch, A)
+    pl.apply_linear(X)
+    got = X.cpu().numpy()
+    E = orc.linear_table(p.M, p.N, p.dt, p.h / 2, p.alpha, p.beta, nthreads=orc.default_threads())
+    want = orc.apply_D(A, E, nthreads=orc.default_threads())
+    err = workloads.rel_l2_per_field(got, want)
+    assert err.max() <= 5e-14, err
+
+
+def test_linear_operator_white_input_all_bins(mmf, torch, orc):
+    """White (all-bin) input exercises every entry of the exp(h/2 L) table including the Nyquist bin."""
+    M, N = 2, 1 << 13
+    p = workloads.problem(4, M=M, N=N)
+    A = rand_c(np.random.default_rng(8), 2 * M, N)
+    pl = plan_for(mmf, p)
+    X = to_dev(torch, A)
+    pl.apply_linear(X)
+    E = orc.linear_table(M, N, p.dt, p.h / 2, p.alpha, p.beta)
+    want = orc.apply_D(A, E)
+    assert workloads.rel_l2_per_field(X.cpu().numpy(), want).max() <= 5e-14
+
+
+# --------------------------------------------------------------------------------------------- nonlinear operator
+@pytest.mark.parametrize("M,N", [(1, 16), (5, 64), (37, 128), (120, 96 * 0 + 256)])
+def test_nonlinear_operator_integer_exact(mmf, torch, orc, M, N):
+    """P10 ii: Gaussian-integer field, integer NON-symmetric kappa, h*gamma = 1: bit-exact against the oracle."""
+    rng = np.random.default_rng(M * 1000 + N)
+    u = rng.integers(-30, 31, size=(2 * M, N)) + 1j * rng.integers(-30, 31, size=(2 * M, N))
+    kap = rng.integers(-9, 10, size=(M, M)).astype(float)
+    pl = mmf.Plan(M, N, 1.0, 1.0, 0.0, np.zeros((M, 1)), 1.0, kap)
+    U = to_dev(torch, u.astype(complex))
+    OUT = torch.empty_like(U)
+    pl.apply_nonlinear(U, OUT)
+    want = orc.nonlinear(u.astype(complex), 1.0, kap)
+    assert np.array_equal(OUT.cpu().numpy(), want)
+    pl.apply_nonlinear(U, U)                        # exact aliasing is allowed
+    assert np.array_equal(U.cpu().numpy(), want)
+
+
+@pytest.mark.parametrize("cfg,M,logn", [(0, 2, 12), (2, 36, 10), (3, 120, 9)])
+def test_nonlinear_operator_matches_oracle(mmf, torch, orc, cfg, M, logn):
+    p = workloads.problem(cfg, M=M, N=1 << logn)
+    A = p.field() * 30.0
+    pl = plan_for(mmf, p)
+    U = to_dev(torch, A)
+    OUT = torch.empty_like(U)
+    pl.apply_nonlinear(U, OUT)
+    want = orc.nonlinear(A, p.h * p.gamma, p.kappa, nthreads=orc.default_threads())
+    assert workloads.rel_l2_per_field(OUT.cpu().numpy(), want).max() <= 1e-14
+
+
+# ----------------------------------------------------------------------------------------------- the RK4IP step
+# (config, M, log2 N, steps): shrunken versions of the five configs of BASELINE.json that the oracle finishes in
+# seconds, spanning single-pass (N <= 4096) and three-pass transforms, ragged mode counts and several time tiles.
+CASES = [
+    (0, 2, 12, 100),      # config 0 at full size and step count
+    (1, 6, 13, 40),
+    (1, 6, 16, 12),       # config 1 at full size, shortened
+    (2, 36, 14, 8),
+    (3, 120, 13, 4),
+    (4, 120, 14, 3),
+    (4, 7, 18, 3),        # config-4 physics at the 2^18 transform size, odd mode count
+]
+
+
+@pytest.mark.parametrize("cfg,M,logn,steps", CASES)
+def test_propagate_matches_oracle(mmf, torch, orc, cfg, M, logn, steps):
+    p = workloads.problem(cfg, M=M, N=1 << logn, steps=steps)
+    A = p.field()
+    pl = plan_for(mmf, p)
+    X = to_dev(torch, A)
+    pl.propagate(X, steps)
+    torch.cuda.synchronize()
+    got = X.cpu().numpy()
+    want = orc.rk4ip(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, steps)
+    err = workloads.rel_l2_per_field(got, want)
+    assert workloads.rel_l2_per_field(want, A).min() > 1e-6          # the propagation did something
+    assert err.max() <= TOL_FIELD, (err.max(), err.argmax())
+
+
+def test_propagate_composes_and_zero_steps(mmf, torch, orc):
+    """mmf_propagate(n1) then (n2) == (n1+n2) (checks the fused next-step bracket); nsteps = 0 is a no-op."""
+    p = workloads.problem(1, M=3, N=1 << 13, steps=5)
+    A = p.field()
+    pl = plan_for(mmf, p)
+    X = to_dev(torch, A)
+    pl.propagate(X, 0)
+    assert np.array_equal(X.cpu().numpy(), A)
+    pl.propagate(X, 5)
+    Y = to_dev(torch, A)
+    pl.propagate(Y, 2)
+    pl.propagate(Y, 3)
+    assert workloads.rel_l2_per_field(Y.cpu().numpy(), X.cpu().numpy()).max() <= 1e-14
+
+
+def test_zero_field_stays_zero(mmf, torch):
+    p = workloads.problem(0, N=1 << 12, steps=3)
+    A = p.field()
+    A[2] = 0
+    pl = plan_for(mmf, p)
+    X = to_dev(torch, A)
+    pl.propagate(X, 3)
+    out = X.cpu().numpy()
+    assert np.all(out[2] == 0) and np.any(out[3] != 0)
+
+
+def test_propagate_host_entry_point(mmf, torch, orc):
+    p = workloads.problem(0, N=1 << 12, steps=4)
+    A = p.field()
+    pl = plan_for(mmf, p)
+    H = torch.from_numpy(A.copy()).pin_memory()
+    scratch = torch.empty((2 * p.M, p.N), dtype=torch.complex128, device="cuda:0")
+    pl.propagate_host(H, scratch, 4)
+    want = orc.rk4ip(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, 4)
+    assert workloads.rel_l2_per_field(H.numpy(), want).max() <= TOL_FIELD
+    assert pl.launch_count() > 0
+
+
+def test_error_paths_on_device(mmf, torch):
+    p = workloads.problem(0, N=1 << 12)
+    pl = plan_for(mmf, p)
+    X = torch.zeros((2 * p.M, p.N), dtype=torch.complex128, device="cuda:0")
+    import ctypes
+    L = mmf.lib()
+    assert L.mmf_propagate(pl._h, ctypes.c_void_p(X.data_ptr()), -1, None) == mmf.MMF_EINVAL
+    assert L.mmf_propagate(pl._h, None, 1, None) == mmf.MMF_EINVAL
+    assert L.mmf_propagate(pl._h, ctypes.c_void_p(X.data_ptr() + 8), 1, None) == mmf.MMF_EINVAL
+    assert L.mmf_plan_set_workspace(pl._h, ctypes.c_void_p(pl._ws_ptr), 16, None) == mmf.MMF_EINVAL
