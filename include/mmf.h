@@ -82,6 +82,16 @@ int mmf_debug_freq_index(mmf_plan *plan, long long *idx_host);
 /* Number of kernel launches this plan has enqueued since creation (bench.py's gpu_launches). */
 long long mmf_plan_launch_count(const mmf_plan *plan);
 
+/* Per-kernel timing for bench.py's roofline.  mmf_plan_set_timing(plan, 1) makes every later launch of
+ * this plan be bracketed by a pair of CUDA events on the launching stream (and drops earlier records); (plan, 0)
+ * switches it off.  mmf_plan_get_timing SYNCHRONISES on the recorded events of kernel class `kclass`
+ * (0 <= kclass < mmf_kernel_class_count()) and returns their summed device time [ms], their number, and the
+ * ALGORITHMIC bytes one such launch moves as mmf_propagate issues it (full-field reads + writes; tables excluded). */
+int mmf_plan_set_timing(mmf_plan *plan, int enable);
+int mmf_kernel_class_count(void);
+const char *mmf_kernel_class_name(int kclass);
+int mmf_plan_get_timing(mmf_plan *plan, int kclass, double *total_ms, long long *launches, double *alg_bytes);
+
 /* Frees the plan and its device tables (not the workspace, which the caller owns). */
 int mmf_plan_destroy(mmf_plan *plan);
 

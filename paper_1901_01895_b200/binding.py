@@ -16,7 +16,8 @@ MMF_OK, MMF_EINVAL, MMF_ENOMEM, MMF_ECUDA = 0, -1, -2, -3
 # every symbol include/mmf.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["mmf_plan_create", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate",
            "mmf_propagate_host", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
-           "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_destroy", "mmf_status_string", "mmf_version"]
+           "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_set_timing", "mmf_kernel_class_count",
+           "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version"]
 
 _lib = None
 
@@ -56,6 +57,14 @@ def lib():
     L.mmf_debug_freq_index.restype = i
     L.mmf_plan_launch_count.argtypes = [vp]
     L.mmf_plan_launch_count.restype = ll
+    L.mmf_plan_set_timing.argtypes = [vp, i]
+    L.mmf_plan_set_timing.restype = i
+    L.mmf_kernel_class_count.argtypes = []
+    L.mmf_kernel_class_count.restype = i
+    L.mmf_kernel_class_name.argtypes = [i]
+    L.mmf_kernel_class_name.restype = ctypes.c_char_p
+    L.mmf_plan_get_timing.argtypes = [vp, i, dp, ctypes.POINTER(ll), dp]
+    L.mmf_plan_get_timing.restype = i
     L.mmf_plan_destroy.argtypes = [vp]
     L.mmf_plan_destroy.restype = i
     L.mmf_status_string.argtypes = [i]
@@ -144,6 +153,22 @@ class Plan:
 
     def launch_count(self):
         return int(lib().mmf_plan_launch_count(self._h))
+
+    def set_timing(self, enable):
+        _check(lib().mmf_plan_set_timing(self._h, 1 if enable else 0), "mmf_plan_set_timing")
+
+    def get_timing(self):
+        """[{name, total_ms, launches, alg_bytes_per_launch}] for every kernel class with at least one launch."""
+        L = lib()
+        out = []
+        for k in range(L.mmf_kernel_class_count()):
+            ms, n, by = ctypes.c_double(), ctypes.c_longlong(), ctypes.c_double()
+            _check(L.mmf_plan_get_timing(self._h, k, ctypes.byref(ms), ctypes.byref(n), ctypes.byref(by)),
+                   "mmf_plan_get_timing")
+            if n.value:
+                out.append(dict(name=L.mmf_kernel_class_name(k).decode(), total_ms=ms.value, launches=n.value,
+                                alg_bytes_per_launch=by.value))
+        return out
 
     def destroy(self):
         if self._h:

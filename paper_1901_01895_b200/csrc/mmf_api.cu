@@ -99,9 +99,44 @@ struct mmf_plan {
   size_t ws_bytes = 0, field_bytes = 0;
   cpx *Y = nullptr, *Z = nullptr, *W = nullptr, *E = nullptr;
   long long launches = 0;
+  // optional per-launch CUDA-event timing (mmf_plan_set_timing): one (start, stop) pair per launch
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;       // 2 per recorded launch
+  std::vector<int> ev_class;         // kernel class of each recorded launch
 };
 
 namespace {
+
+// ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
+enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
+       KC_COUNT };
+const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
+                                        "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>"};
+
+// event bracket around one launch when timing is on (events go on the launching stream)
+struct LaunchTimer {
+  mmf_plan* p;
+  cudaStream_t st;
+  cudaEvent_t stop = nullptr;
+  LaunchTimer(mmf_plan* p_, int kclass, cudaStream_t st_) : p(p_), st(st_) {
+    if (!p->timing) return;
+    cudaEvent_t a = nullptr;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&stop) != cudaSuccess) { stop = nullptr; return; }
+    p->ev.push_back(a);
+    p->ev.push_back(stop);
+    p->ev_class.push_back(kclass);
+    cudaEventRecord(a, st);
+  }
+  ~LaunchTimer() {
+    if (stop) cudaEventRecord(stop, st);
+  }
+};
+
+void clear_events(mmf_plan* p) {
+  for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
+  p->ev.clear();
+  p->ev_class.clear();
+}
 
 // ---- launch helpers ----------------------------------------------------------------------------------------------
 template <int LOGN1, int DIR>
@@ -117,6 +152,7 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   }
   dim3 grid((unsigned)(1u << (p->logn2 - LOGW)), (unsigned)(2 * p->M), (unsigned)nbuf);
   TwoLevelTw tw{p->d_whi, p->d_wlo, p->lb};
+  LaunchTimer lt(p, DIR == 0 ? KC_COLS_FWD : KC_COLS_INV, st);
   kern<<<grid, 1 << (LOGTOT - 4), smem, st>>>(X0, X1, p->d_tw1, tw, p->logn2);
   p->launches++;
   CU(cudaGetLastError());
@@ -150,6 +186,7 @@ int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   }
   const long long nchunks = (2LL * p->M) << p->logn1;
   dim3 grid((unsigned)((nchunks + (1 << LOGB) - 1) >> LOGB), 1, (unsigned)nbuf);
+  LaunchTimer lt(p, KC_ROWS, st);
   kern<<<grid, 1 << (LOGTOT - 4), smem, st>>>(X0, X1, p->E, p->d_tw2, nchunks, p->logn1);
   p->launches++;
   CU(cudaGetLastError());
@@ -199,6 +236,7 @@ int launch_nl(mmf_plan* p, cpx* X, cpx* Y, cpx* Z, cpx* W, cudaStream_t st) {
   q.M = p->M;
   q.N = p->N;
   const unsigned grid = (unsigned)((p->N + MMF_NL_T - 1) / MMF_NL_T);
+  LaunchTimer lt(p, KC_NL_PLAIN + MODE, st);
   kern<<<grid, MMF_NL_T * MMF_NL_WARPS, smem, st>>>(q);
   p->launches++;
   CU(cudaGetLastError());
@@ -212,6 +250,7 @@ bool finite_all(const double* v, size_t n) {
 }
 
 void free_tables(mmf_plan* p) {
+  clear_events(p);
   cudaFree(p->d_kappa);
   cudaFree(p->d_tw1);
   cudaFree(p->d_tw2);
@@ -400,6 +439,45 @@ int mmf_debug_freq_index(mmf_plan* p, long long* idx_host) {
 }
 
 long long mmf_plan_launch_count(const mmf_plan* p) { return p ? p->launches : 0; }
+
+int mmf_plan_set_timing(mmf_plan* p, int enable) {
+  if (!p) return MMF_EINVAL;
+  clear_events(p);
+  p->timing = enable != 0;
+  return MMF_OK;
+}
+
+int mmf_kernel_class_count(void) { return KC_COUNT; }
+
+const char* mmf_kernel_class_name(int kclass) { return (kclass >= 0 && kclass < KC_COUNT) ? kc_names[kclass] : ""; }
+
+int mmf_plan_get_timing(mmf_plan* p, int kclass, double* total_ms, long long* launches, double* alg_bytes) {
+  if (!p || kclass < 0 || kclass >= KC_COUNT || !total_ms || !launches || !alg_bytes) return MMF_EINVAL;
+  double tot = 0.0, bytes = 0.0;
+  long long n = 0;
+  for (size_t i = 0; i < p->ev_class.size(); ++i) {
+    if (p->ev_class[i] != kclass) continue;
+    CU(cudaEventSynchronize(p->ev[2 * i + 1]));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, p->ev[2 * i], p->ev[2 * i + 1]));
+    tot += ms;
+    ++n;
+  }
+  // algorithmic bytes of ONE launch as mmf_propagate issues it: full-field reads + writes
+  const double F = (double)p->field_bytes;
+  switch (kclass) {
+    case KC_COLS_FWD: case KC_ROWS: case KC_COLS_INV: bytes = 4 * F; break;  // two fields, read + write each
+    case KC_NL_PLAIN: bytes = 2 * F; break;
+    case KC_NL_STAGE2: bytes = 3 * F; break;
+    case KC_NL_STAGE3: bytes = 5 * F; break;
+    case KC_NL_FINAL: bytes = 3 * F; break;
+    case KC_NL_FINAL_NEXT: bytes = 4 * F; break;
+  }
+  *total_ms = tot;
+  *launches = n;
+  *alg_bytes = bytes;
+  return MMF_OK;
+}
 
 int mmf_plan_destroy(mmf_plan* p) {
   if (!p) return MMF_EINVAL;
