@@ -8,6 +8,7 @@
 
 #include "../../include/mmf.h"
 #include "kernels.cuh"
+#include "nl_mma.cuh"
 
 using namespace mmf;
 
@@ -89,6 +90,8 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct mmf_plan {
   int M = 0, K = 0, logn = 0, logn1 = 0, logn2 = 0, lb = 0;
+  int nlm_nk = -1;   // k-steps of the tensor-path nonlinear kernel; -1: M too large, legacy kernels (4 buffers)
+  int num_sms = 148;
   long long N = 0;
   double dt = 0, h = 0, alpha = 0, gamma = 0;
   std::vector<double> beta, kappa;
@@ -109,9 +112,10 @@ namespace {
 
 // ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
 enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
-       KC_COUNT };
+       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_COUNT };
 const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
-                                        "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>"};
+                                        "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>", "k_nlm<plain>",
+                                        "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
 struct LaunchTimer {
@@ -243,6 +247,63 @@ int launch_nl(mmf_plan* p, cpx* X, cpx* Y, cpx* Z, cpx* W, cudaStream_t st) {
   return MMF_OK;
 }
 
+// ---- fused nonlinear kernel on the fp64 tensor path (M <= MMF_NLM_MAXM) ------------------------------------------
+constexpr int kNlmNk[] = {1, 2, 3, 4, 6, 8, 9, 12, 16, 20, 24, 28, 30, 32};
+
+int nlm_pick_nk(int M) {
+  const int need = (M + 3) / 4;
+  for (int nk : kNlmNk)
+    if (nk >= need) return nk;
+  return -1;
+}
+
+template <int NK, int MODE>
+int launch_nlm_t(mmf_plan* p, const cpx* U, cpx* X, cpx* Y, cudaStream_t st) {
+  auto kern = k_nlm<NK, MODE>;
+  constexpr int NARR = nlm_narr<MODE>();
+  NlmParams q;
+  q.U = U; q.X = X; q.Y = Y;
+  q.kappa = p->d_kappa;
+  q.hg = p->h * p->gamma;
+  q.M = p->M;
+  q.NW = (p->M + 7) / 8;
+  q.N = p->N;
+  q.ntiles = p->N / MMF_NLM_T;
+  const size_t gsm = nlm_group_smem(p->M, NK, NARR);
+  int tg = 16 / q.NW;                                  // at most 16 warps per CTA (128 registers per thread)
+  const int tg_smem = (int)((size_t)(200 * 1024) / gsm);
+  if (tg > tg_smem) tg = tg_smem;
+  while (tg > 1 && 32 * q.NW * tg > nlm_max_threads(NK)) --tg;   // the kernel's __launch_bounds__
+  if (tg < 1) return MMF_EINVAL;
+  if ((long long)tg > q.ntiles) tg = (int)q.ntiles;
+  q.TG = tg;
+  const size_t smem = gsm * tg;
+  static size_t attr_smem = 0;
+  if (smem > attr_smem) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_smem = smem;
+  }
+  long long grid = (q.ntiles + tg - 1) / tg;
+  if (grid > p->num_sms) grid = p->num_sms;            // persistent: one CTA per SM
+  LaunchTimer lt(p, KC_NLM_PLAIN + MODE, st);
+  kern<<<(unsigned)grid, 32 * q.NW * tg, smem, st>>>(q);
+  p->launches++;
+  CU(cudaGetLastError());
+  return MMF_OK;
+}
+
+template <int MODE>
+int launch_nlm(mmf_plan* p, const cpx* U, cpx* X, cpx* Y, cudaStream_t st) {
+  switch (p->nlm_nk) {
+#define MMF_NLM_CASE(NKV) case NKV: return launch_nlm_t<NKV, MODE>(p, U, X, Y, st);
+    MMF_NLM_CASE(1) MMF_NLM_CASE(2) MMF_NLM_CASE(3) MMF_NLM_CASE(4) MMF_NLM_CASE(6) MMF_NLM_CASE(8) MMF_NLM_CASE(9)
+    MMF_NLM_CASE(12) MMF_NLM_CASE(16) MMF_NLM_CASE(20) MMF_NLM_CASE(24) MMF_NLM_CASE(28) MMF_NLM_CASE(30)
+    MMF_NLM_CASE(32)
+#undef MMF_NLM_CASE
+    default: return MMF_EINVAL;
+  }
+}
+
 bool finite_all(const double* v, size_t n) {
   for (size_t i = 0; i < n; ++i)
     if (!std::isfinite(v[i])) return false;
@@ -301,6 +362,13 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
     p->logn1 = logn - p->logn2;
   }
   p->lb = (logn + 1) / 2;
+  p->nlm_nk = (M <= MMF_NLM_MAXM) ? nlm_pick_nk(M) : -1;
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      p->num_sms = sms;
+  }
   p->field_bytes = sizeof(cpx) * 2 * (size_t)M * (size_t)N;
   int rc = MMF_OK;
   do {
@@ -341,7 +409,7 @@ size_t mmf_plan_workspace_bytes(const mmf_plan* p) {
   if (!p) return 0;
   const size_t F = align_up(p->field_bytes, 256);
   const size_t E = align_up(sizeof(cpx) * (size_t)p->M * (size_t)p->N, 256);
-  return 3 * F + E;
+  return (p->nlm_nk > 0 ? 1 : 3) * F + E;
 }
 
 int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_stream) {
@@ -352,9 +420,14 @@ int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_s
   p->ws = (unsigned char*)ws_dev;
   p->ws_bytes = bytes;
   p->Y = (cpx*)(p->ws);
-  p->Z = (cpx*)(p->ws + F);
-  p->W = (cpx*)(p->ws + 2 * F);
-  p->E = (cpx*)(p->ws + 3 * F);
+  if (p->nlm_nk > 0) {
+    p->Z = p->W = nullptr;
+    p->E = (cpx*)(p->ws + F);
+  } else {
+    p->Z = (cpx*)(p->ws + F);
+    p->W = (cpx*)(p->ws + 2 * F);
+    p->E = (cpx*)(p->ws + 3 * F);
+  }
   EtabParams P;
   memset(&P, 0, sizeof(P));
   static const dd TWO_PI_DD = {6.283185307179586232e+00, 2.449293598294706414e-16};
@@ -378,6 +451,19 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cpx *X = (cpx*)A_dev, *Y = p->Y, *Z = p->Z, *W = p->W;
   int rc;
+  if (p->nlm_nk > 0) {
+    // two full-field buffers: X (the caller's field) and Y.  Per step: D(X,Y); S23 in place; D(X,Y); FINAL(+NEXT).
+    if ((rc = launch_nlm<NLM_PLAIN>(p, X, Y, nullptr, st)) != MMF_OK) return rc;   // Y <- h N(A) A   (6b bracket)
+    for (int s = 0; s < nsteps; ++s) {
+      if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6a) A_I, (6b) k1
+      if ((rc = launch_nlm<NLM_S23>(p, nullptr, X, Y, st)) != MMF_OK) return rc;    // (6c), (6d), brackets of 6e/6f
+      if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6e) argument, (6f) first term
+      if (s + 1 < nsteps) rc = launch_nlm<NLM_FINAL_NEXT>(p, nullptr, X, Y, st);    // (6e)+(6f), next (6b) bracket
+      else rc = launch_nlm<NLM_FINAL>(p, nullptr, X, Y, st);
+      if (rc != MMF_OK) return rc;
+    }
+    return MMF_OK;
+  }
   // the bracket of Eq. (6b) for the first step; later steps get it from NL_FINAL_NEXT
   if ((rc = launch_nl<NL_PLAIN>(p, X, Y, Z, W, st)) != MMF_OK) return rc;
   for (int s = 0; s < nsteps; ++s) {
@@ -410,6 +496,7 @@ int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
 
 int mmf_apply_nonlinear(mmf_plan* p, const void* U_dev, void* OUT_dev, void* cuda_stream) {
   if (!p || !U_dev || !OUT_dev || (((size_t)U_dev | (size_t)OUT_dev) & 15) != 0) return MMF_EINVAL;
+  if (p->nlm_nk > 0) return launch_nlm<NLM_PLAIN>(p, (const cpx*)U_dev, (cpx*)OUT_dev, nullptr, (cudaStream_t)cuda_stream);
   return launch_nl<NL_PLAIN>(p, (cpx*)U_dev, (cpx*)OUT_dev, nullptr, nullptr, (cudaStream_t)cuda_stream);
 }
 
@@ -472,6 +559,10 @@ int mmf_plan_get_timing(mmf_plan* p, int kclass, double* total_ms, long long* la
     case KC_NL_STAGE3: bytes = 5 * F; break;
     case KC_NL_FINAL: bytes = 3 * F; break;
     case KC_NL_FINAL_NEXT: bytes = 4 * F; break;
+    case KC_NLM_PLAIN: bytes = 2 * F; break;
+    case KC_NLM_S23: bytes = 4 * F; break;
+    case KC_NLM_FINAL: bytes = 3 * F; break;
+    case KC_NLM_FINAL_NEXT: bytes = 4 * F; break;
   }
   *total_ms = tot;
   *launches = n;
