@@ -2,14 +2,21 @@
 //
 // Role in the path: rows a1/a3 of the hot-path table (forward / inverse transform of every field, PAPER.md:107
 // "fast Fourier transforms ... rows are aligned linear in the memory"; Eq. 6 PAPER.md:75-88 needs exp(h/2 L)
-// four times per step).  Design (DESIGN.md §FFT):
-//   * every thread owns 16 complex values (64 registers) and performs radix-2..16 butterflies on them;
-//   * a tile of 2^LOGTOT complex values lives in shared memory; one "stage" reads 16 values per thread,
-//     transforms one digit of the index and writes them back IN PLACE (decimation in frequency on the way to
-//     the spectrum, the exact adjoint — decimation in time — on the way back), so no bit-reversal pass exists:
-//     the spectrum simply stays in digit-reversed slot order and the exp(h/2 L) table is stored in that order;
-//   * the 16 values a thread touches always span 4 contiguous index bits and the tile is XOR-swizzled
-//     (slot ^ ((slot >> 4) & 7)) which makes every stage's LDS.128/STS.128 pattern bank-conflict free.
+// four times per step).  Design (DESIGN.md "Kernels"):
+//   * a "tile" is 2^12 complex values worked on by one GROUP of 256 threads; every thread owns 16 values
+//     (64 registers) and performs radix-2..16 butterflies on them;
+//   * a transform of 2^LOGP points is split into NST = ceil(LOGP/4) digits.  The FIRST stage takes its 16 values
+//     straight from global memory and the LAST stage leaves them in registers for the epilogue (spectral multiply,
+//     inter-pass twiddle, store): shared memory is only the exchange buffer BETWEEN stages (one STS.128 + one
+//     LDS.128 per value per exchange, one group barrier per exchange);
+//   * decimation in frequency on the way to the spectrum, the exact adjoint (decimation in time) on the way back,
+//     so no bit-reversal pass exists: the spectrum stays in digit-reversed slot order, the last forward stage and
+//     the first inverse stage share one register layout, and the exp(h/2 L) table is stored in that order;
+//   * the exchange buffer is XOR-swizzled (slot ^ ((slot >> 4) & 7)): every stage's LDS.128/STS.128 pattern is
+//     bank-conflict free;
+//   * inter-stage twiddles come from per-stage tables laid out [c][b] (c = output index of the butterfly, b = low
+//     bits of the point index): lanes read consecutive or identical entries, one to four wavefronts per load
+//     instead of a 32-way gather from a length-N table.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -81,12 +88,22 @@ struct Dft<1, SIGN> {
   static __device__ __forceinline__ void run(cpx (&)[1]) {}
 };
 
-__device__ __forceinline__ int swz(int f) { return f ^ ((f >> 4) & 7); }
+#define MMF_TILE_LOG 12        // complex values per group tile (2^12 = 64 KiB of exchange buffer)
+#define MMF_GROUP_THREADS 256  // 2^(MMF_TILE_LOG - 4)
+
+__host__ __device__ __forceinline__ constexpr int swz(int f) { return f ^ ((f >> 4) & 7); }
 
 // Split of a length-2^LOGN transform into NST = ceil(LOGN/4) digits, most significant first:
 // digit i has LR = ceil(remaining / stages_left) bits.
 __host__ __device__ constexpr int nstages(int logn) { return (logn + 3) / 4; }
 __host__ __device__ constexpr int stage_lr(int remain, int nst) { return (remain + nst - 1) / nst; }
+// digit widths of the last and the last-but-one stage
+__host__ __device__ constexpr int last_lr(int remain, int nst) {
+  return nst <= 1 ? remain : last_lr(remain - stage_lr(remain, nst), nst - 1);
+}
+__host__ __device__ constexpr int prev_lr(int remain, int nst) {
+  return nst <= 1 ? 0 : nst == 2 ? stage_lr(remain, 2) : prev_lr(remain - stage_lr(remain, nst), nst - 1);
+}
 
 // Slot p (digits d1 d2 ... most significant first, radices r1 r2 ...) holds bin k = d1 + r1 d2 + r1 r2 d3 + ...
 template <int REMAIN, int NST>
@@ -104,23 +121,57 @@ __host__ __device__ __forceinline__ constexpr int slot_to_bin(int p) {
   return slot_to_bin<LOGN, nstages(LOGN)>(p);
 }
 
-// One in-place stage on a shared-memory tile of 2^LOGTOT values = 2^(LOGTOT-LOGW) transform points x 2^LOGW
-// interleaved columns.  Transforms the LR-bit digit sitting at point-index bits [LOGM+LR-1 : LOGM].
-//   DIF:  v <- Dft(v) then v[c] *= w_L^(SIGN b c)        (L = 2^(LR+LOGM), b = point index mod 2^LOGM)
-//   DIT:  v[c] *= w_L^(SIGN b c) then v <- Dft(v)        (the adjoint of the DIF stage of opposite SIGN)
-// tw[] holds exp(+2 pi i j / 2^LOGN) for j < 2^LOGN (LOGN = transform length; tile bits above LOGN + LOGW are a
-// batch index).  t = thread index in [0, 2^(LOGTOT-4)).
-template <int LOGTOT, int LOGN, int LOGW, int LOGM, int LR, int SIGN, bool DIF>
-__device__ __forceinline__ void smem_stage(cpx* __restrict__ s, int t, const cpx* __restrict__ tw) {
-  constexpr int SH = LOGM + LOGW;
-  constexpr int LO = (SH < LOGTOT - 4) ? SH : (LOGTOT - 4);
-  constexpr int R = 1 << LR;
-  constexpr int DSH = SH - LO;
-  constexpr int TWSH = LOGN - LR - LOGM;
-  const int base = ((t >> LO) << (LO + 4)) | (t & ((1 << LO) - 1));
-  cpx v[16];
+// ---- per-stage twiddle tables ---------------------------------------------------------------------------------------
+// The stage that transforms an LR-bit digit with LOGM point-index bits below it multiplies output c of the
+// butterfly at low index b by exp(+-2 pi i b c / 2^(LR+LOGM)).  Table of one stage: entry [(c-1) << LOGM | b],
+// c = 1 .. 2^LR - 1, b < 2^LOGM (stages with LOGM = 0 have none).  Tables of all stages are concatenated, most
+// significant digit first.  (The host fills them with the same recursion, mmf_api.cu.)
+__host__ __device__ constexpr int tw_stage_entries(int lr, int logm) { return logm > 0 ? (((1 << lr) - 1) << logm) : 0; }
+__host__ __device__ constexpr int tw_total_entries(int remain, int nst) {
+  return nst <= 0 ? 0
+                  : tw_stage_entries(stage_lr(remain, nst), remain - stage_lr(remain, nst)) +
+                        tw_total_entries(remain - stage_lr(remain, nst), nst - 1);
+}
+__host__ __device__ constexpr int tw_offset(int logp, int remain, int nst) {
+  return tw_total_entries(logp, nstages(logp)) - tw_total_entries(remain, nst);
+}
+
+// ---- register layout of a stage -------------------------------------------------------------------------------------
+// A tile is 2^LOGTOT values = [batch][point (LOGP bits)][column (LOGW bits)], flat index f.  In the stage whose digit
+// sits at point bits [LOGM+LR-1 : LOGM], thread t owns f_j = base | (j << LO), j = 0..15, with
+// LO = min(LOGM + LOGW, LOGTOT - 4) and base = t with four zero bits inserted at position LO.
+__host__ __device__ constexpr int stage_lo(int logm, int logw, int logtot) {
+  return (logm + logw < logtot - 4) ? (logm + logw) : (logtot - 4);
+}
+template <int LO>
+__device__ __forceinline__ int stage_base(int t) {
+  return ((t >> LO) << (LO + 4)) | (t & ((1 << LO) - 1));
+}
+template <int LO>
+__device__ __forceinline__ void tile_lds(cpx (&v)[16], const cpx* __restrict__ s, int base) {
 #pragma unroll
   for (int j = 0; j < 16; ++j) v[j] = s[swz(base | (j << LO))];
+}
+template <int LO>
+__device__ __forceinline__ void tile_sts(const cpx (&v)[16], cpx* __restrict__ s, int base) {
+#pragma unroll
+  for (int j = 0; j < 16; ++j) s[swz(base | (j << LO))] = v[j];
+}
+
+__device__ __forceinline__ void group_barrier(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// One stage on the 16 registers of a thread.
+//   DIF:  x <- Dft(x) then x[c] *= w_L^(SIGN b c)        (L = 2^(LR+LOGM), b = point index mod 2^LOGM)
+//   DIT:  x[c] *= w_L^(SIGN b c) then x <- Dft(x)        (the adjoint of the DIF stage of opposite SIGN)
+// tab = this stage's twiddle table (see above), exp(+2 pi i b c / L).
+template <int LOGTOT, int LOGW, int LOGM, int LR, int SIGN, bool DIF>
+__device__ __forceinline__ void stage_math(cpx (&v)[16], int base, const cpx* __restrict__ tab) {
+  constexpr int SH = LOGM + LOGW;
+  constexpr int LO = stage_lo(LOGM, LOGW, LOGTOT);
+  constexpr int R = 1 << LR;
+  constexpr int DSH = SH - LO;
 #pragma unroll
   for (int q = 0; q < 16 / R; ++q) {
     const int jq = ((q >> DSH) << (DSH + LR)) | (q & ((1 << DSH) - 1));
@@ -132,41 +183,56 @@ __device__ __forceinline__ void smem_stage(cpx* __restrict__ s, int t, const cpx
       Dft<R, SIGN>::run(x);
       if constexpr (LOGM > 0) {
 #pragma unroll
-        for (int c = 1; c < R; ++c) x[c] = cmul_s<SIGN>(x[c], tw[(b * c) << TWSH]);
+        for (int c = 1; c < R; ++c) x[c] = cmul_s<SIGN>(x[c], tab[((c - 1) << LOGM) | b]);
       }
     } else {
       if constexpr (LOGM > 0) {
 #pragma unroll
-        for (int c = 1; c < R; ++c) x[c] = cmul_s<SIGN>(x[c], tw[(b * c) << TWSH]);
+        for (int c = 1; c < R; ++c) x[c] = cmul_s<SIGN>(x[c], tab[((c - 1) << LOGM) | b]);
       }
       Dft<R, SIGN>::run(x);
     }
 #pragma unroll
     for (int a = 0; a < R; ++a) v[jq | (a << DSH)] = x[a];
   }
-#pragma unroll
-  for (int j = 0; j < 16; ++j) s[swz(base | (j << LO))] = v[j];
 }
 
-// All stages, most significant digit first (DIF, natural order in -> digit-reversed slots out) ...
-template <int LOGTOT, int LOGN, int LOGW, int REMAIN, int NST, int SIGN>
-__device__ __forceinline__ void smem_fft_dif(cpx* s, int t, const cpx* __restrict__ tw) {
-  if constexpr (NST > 0) {
-    constexpr int LR = stage_lr(REMAIN, NST);
-    smem_stage<LOGTOT, LOGN, LOGW, REMAIN - LR, LR, SIGN, true>(s, t, tw);
-    __syncthreads();
-    smem_fft_dif<LOGTOT, LOGN, LOGW, REMAIN - LR, NST - 1, SIGN>(s, t, tw);
+// Forward chain (DIF, most significant digit first).  Entry: v in the layout of stage (REMAIN, NST) — for the first
+// call REMAIN = LOGP, NST = nstages(LOGP), loaded by the caller from global memory.  Exit: v in the layout of the
+// last stage (LOGM = 0), values in digit-reversed slot order.  s = this group's exchange buffer, tab = the
+// concatenated tables of the LOGP-point transform, bar = the group's named-barrier id.
+// FENCE: also synchronise after the last exchange read (needed when the caller's next use of the buffer does not
+// start with the slots this thread read last, i.e. when the chain is not followed by its adjoint).
+template <int LOGTOT, int LOGP, int LOGW, int REMAIN, int NST, int SIGN, bool FENCE>
+__device__ __forceinline__ void fft_dif(cpx (&v)[16], cpx* __restrict__ s, int t, const cpx* __restrict__ tab, int bar) {
+  constexpr int LR = stage_lr(REMAIN, NST), LOGM = REMAIN - LR, LO = stage_lo(LOGM, LOGW, LOGTOT);
+  const int base = stage_base<LO>(t);
+  stage_math<LOGTOT, LOGW, LOGM, LR, SIGN, true>(v, base, tab + tw_offset(LOGP, REMAIN, NST));
+  if constexpr (NST > 1) {
+    constexpr int LR2 = stage_lr(LOGM, NST - 1), LO2 = stage_lo(LOGM - LR2, LOGW, LOGTOT);
+    tile_sts<LO>(v, s, base);
+    group_barrier(bar, MMF_GROUP_THREADS);
+    tile_lds<LO2>(v, s, stage_base<LO2>(t));
+    if constexpr (FENCE && NST == 2) group_barrier(bar, MMF_GROUP_THREADS);
+    fft_dif<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, FENCE>(v, s, t, tab, bar);
   }
 }
-// ... and least significant digit first (DIT, digit-reversed slots in -> natural order out).
-template <int LOGTOT, int LOGN, int LOGW, int REMAIN, int NST, int SIGN>
-__device__ __forceinline__ void smem_fft_dit(cpx* s, int t, const cpx* __restrict__ tw) {
-  if constexpr (NST > 0) {
-    constexpr int LR = stage_lr(REMAIN, NST);
-    smem_fft_dit<LOGTOT, LOGN, LOGW, REMAIN - LR, NST - 1, SIGN>(s, t, tw);
-    smem_stage<LOGTOT, LOGN, LOGW, REMAIN - LR, LR, SIGN, false>(s, t, tw);
-    __syncthreads();
+
+// Inverse chain (DIT, least significant digit first): the adjoint of fft_dif with the opposite SIGN.  Entry: v in the
+// layout of the last stage; exit: v in the layout of stage (REMAIN, NST) of the outermost call, natural order.
+template <int LOGTOT, int LOGP, int LOGW, int REMAIN, int NST, int SIGN, bool FENCE>
+__device__ __forceinline__ void fft_dit(cpx (&v)[16], cpx* __restrict__ s, int t, const cpx* __restrict__ tab, int bar) {
+  constexpr int LR = stage_lr(REMAIN, NST), LOGM = REMAIN - LR, LO = stage_lo(LOGM, LOGW, LOGTOT);
+  const int base = stage_base<LO>(t);
+  if constexpr (NST > 1) {
+    constexpr int LR2 = stage_lr(LOGM, NST - 1), LO2 = stage_lo(LOGM - LR2, LOGW, LOGTOT);
+    fft_dit<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, false>(v, s, t, tab, bar);
+    tile_sts<LO2>(v, s, stage_base<LO2>(t));
+    group_barrier(bar, MMF_GROUP_THREADS);
+    tile_lds<LO>(v, s, base);
+    if constexpr (FENCE) group_barrier(bar, MMF_GROUP_THREADS);
   }
+  stage_math<LOGTOT, LOGW, LOGM, LR, SIGN, false>(v, base, tab + tw_offset(LOGP, REMAIN, NST));
 }
 
 }  // namespace mmf

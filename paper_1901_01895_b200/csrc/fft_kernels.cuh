@@ -1,0 +1,316 @@
+// fft_kernels.cuh — the transform kernels of the RK4IP hot path (sm_100a, fp64): rows a1-a3 of the hot-path table.
+//
+//   k_cols  passes A and C of the three-pass operator D = exp(h/2 L) (Eq. 6a):  length-N1 transforms
+//           over the slow (strided) index of a row viewed as an N1 x N2 matrix, plus the inter-pass twiddle
+//           W_N^(k1 n2).
+//   k_rows  pass B: contiguous length-N2 transform -> multiply by the tabulated exp(h/2 L_a(w_k))/N -> adjoint
+//           length-N2 transform, the spectrum never leaving the SM.  For N <= 4096 this kernel alone is D.
+//   k_etab  fills the exp(h/2 L_a(w_k)) table in the order pass B consumes it (double-double phase).
+//
+// Index algebra of D (forward sign +, reading R1 of DESIGN.md):  n = N2 n1 + n2,  k = k1 + N1 k2,
+//   X[k1 + N1 k2] = sum_n2 W_N2^(k2 n2) [ W_N^(k1 n2) sum_n1 W_N1^(k1 n1) x[N2 n1 + n2] ]
+// pass A does the inner sum and the twiddle, pass B the outer sum; the way back is the exact adjoint.
+//
+// Execution model: persistent CTAs (one per SM) of G independent groups of 256 threads.  A group owns one 64 KiB
+// exchange buffer and walks its own list of 4096-point tiles (fft_core.cuh); groups of a CTA share the stage
+// twiddle tables in shared memory and run out of phase, so that one group's global loads overlap the other's
+// butterflies.  Global loads go straight into the registers of the first stage and the last stage stores from
+// registers.
+#pragma once
+#include "fft_core.cuh"
+
+namespace mmf {
+
+// runtime version of slot_to_bin<LOGN> (same digit rule), used by table generation and the debug map
+__host__ __device__ inline int slot_to_bin_rt(int logn, int p) {
+  int remain = logn, nst = nstages(logn), k = 0, shift = 0;
+  while (nst > 0) {
+    const int lr = stage_lr(remain, nst), lm = remain - lr;
+    k += (p >> lm) << shift;
+    p &= (1 << lm) - 1;
+    shift += lr;
+    remain = lm;
+    --nst;
+  }
+  return k;
+}
+
+__device__ __forceinline__ cpx ld_stream(const cpx* p) { return __ldcs(p); }
+__device__ __forceinline__ void st_stream(cpx* p, cpx v) { __stcs(p, v); }
+
+// copy the stage tables of a transform into shared memory (whole CTA), then synchronise
+template <int ENTRIES>
+__device__ __forceinline__ void load_stage_tables(cpx* __restrict__ tab, const cpx* __restrict__ src) {
+  for (int i = threadIdx.x; i < ENTRIES; i += blockDim.x) tab[i] = src[i];
+  __syncthreads();
+}
+
+// ---------------------------------------------------------------------------------------------------- pass A / C
+struct ColsParams {
+  cpx* X0;
+  cpx* X1;
+  const cpx* __restrict__ twtab;  // stage tables of the N1-point transform
+  const cpx* __restrict__ whi;    // W_N^x = whi[x >> lb] * wlo[x & (2^lb - 1)]
+  const cpx* __restrict__ wlo;
+  const cpx* __restrict__ colA;   // [N2]  W_N^(wA n2): step of register bit 0 of the last-stage layout
+  const cpx* __restrict__ colB;   // [N2]  W_N^(wB n2): step of register bit 3
+  int lb, logn2, nrows, nbuf;
+};
+
+// v[j] *= W_N^(k1(pos0 + j) n2)  (or its conjugate): k1(pos0 + j) = k1(pos0) + wA (j & 7) + wB (j >> 3), so the 16
+// factors are t0 sA^(j&7) sB^(j>>3) — three table look-ups per thread and short product chains (depth <= 4)
+// instead of 32 gathers.
+template <int LOGN1, bool CONJ>
+__device__ __forceinline__ void apply_interpass(cpx (&v)[16], int pos0, long long n2, const ColsParams& p) {
+  const long long x = (long long)slot_to_bin<LOGN1>(pos0) * n2;
+  const cpx t0 = cmul(p.whi[x >> p.lb], p.wlo[x & ((1LL << p.lb) - 1)]);
+  const cpx sA = p.colA[n2];
+  const cpx t1 = cmul(t0, p.colB[n2]);
+  cpx pw[8];
+  pw[1] = sA;
+  pw[2] = cmul(sA, sA);
+  pw[3] = cmul(pw[2], sA);
+  pw[4] = cmul(pw[2], pw[2]);
+  pw[5] = cmul(pw[4], sA);
+  pw[6] = cmul(pw[4], pw[2]);
+  pw[7] = cmul(pw[4], pw[3]);
+  v[0] = CONJ ? cmulc(v[0], t0) : cmul(v[0], t0);
+  v[8] = CONJ ? cmulc(v[8], t1) : cmul(v[8], t1);
+#pragma unroll
+  for (int e = 1; e < 8; ++e) {
+    const cpx a = cmul(t0, pw[e]), b = cmul(t1, pw[e]);
+    v[e] = CONJ ? cmulc(v[e], a) : cmul(v[e], a);
+    v[8 + e] = CONJ ? cmulc(v[8 + e], b) : cmul(v[8 + e], b);
+  }
+}
+
+// grid = persistent (<= one CTA per SM); block = 256 G.  DIR 0: pass A (DIF, sign +, then twiddle);
+// DIR 1: pass C (conjugate twiddle, then DIT, sign -).  A tile is N1 points x W = 2^(12 - LOGN1) adjacent columns.
+// dynamic shared memory: stage tables + G exchange buffers.
+template <int LOGN1, int DIR, int G>
+__global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_cols(ColsParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int LOGW = MMF_TILE_LOG - LOGN1, W = 1 << LOGW;
+  constexpr int NST = nstages(LOGN1);
+  constexpr int TWN = tw_total_entries(LOGN1, NST);
+  constexpr int LR1 = stage_lr(LOGN1, NST), LO1 = stage_lo(LOGN1 - LR1, LOGW, MMF_TILE_LOG);  // first-stage layout
+  constexpr int LOL = stage_lo(0, LOGW, MMF_TILE_LOG);                                        // last-stage layout
+  cpx* tab = reinterpret_cast<cpx*>(smem_raw);
+  load_stage_tables<TWN>(tab, p.twtab);
+  const int grp = threadIdx.x / MMF_GROUP_THREADS, t = threadIdx.x % MMF_GROUP_THREADS;
+  cpx* s = tab + ((TWN + 7) & ~7) + (grp << MMF_TILE_LOG);
+  const int bar = 1 + grp;
+  const int logn2 = p.logn2;
+  const long long N = 1LL << (LOGN1 + logn2);
+  const long long nct = 1LL << (logn2 - LOGW);
+  const long long total = nct * p.nrows * p.nbuf;
+  const int base1 = stage_base<LO1>(t), basel = stage_base<LOL>(t);
+  const int pos0 = basel >> LOGW, c = t & (W - 1);
+  for (long long u = (long long)blockIdx.x * G + grp; u < total; u += (long long)gridDim.x * G) {
+    const long long ct = u & (nct - 1), rb = u >> (logn2 - LOGW);
+    const int row = (int)(rb % p.nrows), buf = (int)(rb / p.nrows);
+    cpx* g = (buf ? p.X1 : p.X0) + (long long)row * N + (ct << LOGW);
+    cpx v[16];
+    if constexpr (DIR == 0) {
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const int f = base1 | (j << LO1);
+        v[j] = ld_stream(g + (((long long)(f >> LOGW)) << logn2) + (f & (W - 1)));
+      }
+      fft_dif<MMF_TILE_LOG, LOGN1, LOGW, LOGN1, NST, +1, true>(v, s, t, tab, bar);
+      apply_interpass<LOGN1, false>(v, pos0, (ct << LOGW) + c, p);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) st_stream(g + (((long long)(pos0 + j)) << logn2) + c, v[j]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < 16; ++j) v[j] = ld_stream(g + (((long long)(pos0 + j)) << logn2) + c);
+      apply_interpass<LOGN1, true>(v, pos0, (ct << LOGW) + c, p);
+      fft_dit<MMF_TILE_LOG, LOGN1, LOGW, LOGN1, NST, -1, true>(v, s, t, tab, bar);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const int f = base1 | (j << LO1);
+        st_stream(g + (((long long)(f >> LOGW)) << logn2) + (f & (W - 1)), v[j]);
+      }
+    }
+  }
+}
+
+// -------------------------------------------------------------------------------------------------------- pass B
+// A "chunk" is one contiguous run of N2 values (memory row p1 of field row r: chunk = r * N1 + p1); a tile is
+// 2^(12 - LOGN2) consecutive chunks.  The exp(h/2 L) table holds, per (mode, p1) chunk, its N2 entries in the
+// register order of the last forward stage: entry [(q & 15) << (LOGN2 - 4) | (q >> 4)] belongs to slot q, so that
+// lanes read consecutive entries.
+struct RowsParams {
+  cpx* X0;
+  cpx* X1;
+  const cpx* __restrict__ E;
+  const cpx* __restrict__ twtab;  // stage tables of the N2-point transform
+  long long nchunks;              // per buffer: 2 M N1
+  int logn1, nbuf, M;
+};
+
+// MODE 0: transform, * E, adjoint transform (in place).  MODE 1: forward transform only, output in slot order
+// (debug entry point).  SINGLE: N1 = 1 (the whole of D in this kernel; tiles may be ragged and hold several rows).
+// Three-pass order of work: an item is (mode a, tile of chunks), its 2 nbuf sub-tiles (polarisation x buffer) share
+// one piece of the table and are done back to back by the same group, so the table is read from HBM once.
+template <int LOGN2, int MODE, bool SINGLE, int G>
+__global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int LOGB = MMF_TILE_LOG - LOGN2;
+  constexpr int NST = nstages(LOGN2);
+  constexpr int TWN = tw_total_entries(LOGN2, NST);
+  constexpr int LR1 = stage_lr(LOGN2, NST), LO1 = stage_lo(LOGN2 - LR1, 0, MMF_TILE_LOG);
+  cpx* tab = reinterpret_cast<cpx*>(smem_raw);
+  load_stage_tables<TWN>(tab, p.twtab);
+  const int grp = threadIdx.x / MMF_GROUP_THREADS, t = threadIdx.x % MMF_GROUP_THREADS;
+  cpx* s = tab + ((TWN + 7) & ~7) + (grp << MMF_TILE_LOG);
+  const int bar = 1 + grp;
+  const int base1 = stage_base<LO1>(t);
+  const int cht = (t << 4) >> LOGN2;                 // chunk (inside the tile) of this thread's last-stage values
+  const int tq = t & ((1 << (LOGN2 - 4)) - 1);
+  const int logn1 = p.logn1;
+  const int sub = SINGLE ? p.nbuf : 2 * p.nbuf;
+  const long long items = SINGLE ? ((p.nchunks + (1 << LOGB) - 1) >> LOGB) : ((long long)p.M << (logn1 - LOGB));
+  for (long long item = (long long)blockIdx.x * G + grp; item < items; item += (long long)gridDim.x * G) {
+    for (int sidx = 0; sidx < sub; ++sidx) {
+      long long chunk0, ech;   // first chunk of the tile; table chunk of this thread's last-stage values
+      int buf;
+      if constexpr (SINGLE) {
+        chunk0 = item << LOGB;
+        buf = sidx;
+        ech = (chunk0 + cht) >> 1;  // chunk = row, table chunk = mode
+      } else {
+        const long long a = item >> (logn1 - LOGB), tau = item & ((1LL << (logn1 - LOGB)) - 1);
+        chunk0 = ((2 * a + (sidx & 1)) << logn1) + (tau << LOGB);
+        buf = sidx >> 1;
+        ech = (a << logn1) + (tau << LOGB) + cht;
+      }
+      cpx* g = (buf ? p.X1 : p.X0) + (chunk0 << LOGN2);
+      cpx v[16];
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const int f = base1 | (j << LO1);
+        const bool live = !SINGLE || chunk0 + (f >> LOGN2) < p.nchunks;
+        v[j] = live ? ld_stream(g + f) : make_double2(0.0, 0.0);
+      }
+      fft_dif<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, +1, MODE == 1>(v, s, t, tab, bar);
+      if constexpr (MODE == 0) {
+        if (!SINGLE || chunk0 + cht < p.nchunks) {
+          const cpx* e = p.E + (ech << LOGN2) + tq;
+#pragma unroll
+          for (int j = 0; j < 16; ++j) v[j] = cmul(v[j], __ldg(e + (j << (LOGN2 - 4))));
+        }
+        fft_dit<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, -1, false>(v, s, t, tab, bar);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          const int f = base1 | (j << LO1);
+          if (!SINGLE || chunk0 + (f >> LOGN2) < p.nchunks) st_stream(g + f, v[j]);
+        }
+      } else {
+        if (!SINGLE || chunk0 + cht < p.nchunks) {
+#pragma unroll
+          for (int j = 0; j < 16; ++j) g[(t << 4) + j] = v[j];
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------- exp(h/2 L) table, slot order
+// double-double helpers (error-free transformations; ~106-bit phase so that the reduced angle is exact to fp64)
+struct dd {
+  double hi, lo;
+};
+__host__ __device__ inline dd dd_quick(double a, double b) {
+  const double s = a + b;
+  return dd{s, b - (s - a)};
+}
+__host__ __device__ inline dd dd_two_sum(double a, double b) {
+  const double s = a + b, bb = s - a;
+  return dd{s, (a - (s - bb)) + (b - bb)};
+}
+__host__ __device__ inline dd dd_two_prod(double a, double b) {
+  const double p = a * b;
+  return dd{p, fma(a, b, -p)};
+}
+__host__ __device__ inline dd dd_add(dd a, dd b) {
+  dd s = dd_two_sum(a.hi, b.hi);
+  dd t = dd_two_sum(a.lo, b.lo);
+  s.lo += t.hi;
+  s = dd_quick(s.hi, s.lo);
+  s.lo += t.lo;
+  return dd_quick(s.hi, s.lo);
+}
+__host__ __device__ inline dd dd_mul(dd a, dd b) {
+  dd p = dd_two_prod(a.hi, b.hi);
+  p.lo += a.hi * b.lo + a.lo * b.hi;
+  return dd_quick(p.hi, p.lo);
+}
+__host__ __device__ inline dd dd_mul_d(dd a, double b) {
+  dd p = dd_two_prod(a.hi, b);
+  p.lo += a.lo * b;
+  return dd_quick(p.hi, p.lo);
+}
+__host__ __device__ inline dd dd_div_d(dd a, double b) {
+  const double q1 = a.hi / b;
+  dd r = dd_add(a, dd_mul_d(dd{-q1, 0.0}, b));
+  const double q2 = r.hi / b;
+  r = dd_add(r, dd_mul_d(dd{-q2, 0.0}, b));
+  const double q3 = r.hi / b;
+  dd q = dd_quick(q1, q2);
+  return dd_add(q, dd{q3, 0.0});
+}
+
+#define MMF_MAXK 8
+struct EtabParams {
+  dd wstep;    // 2 pi / (N dt)
+  dd twopi;
+  double amp;  // exp(-alpha hh / 2) / N
+  int K, logn1, logn2;
+};
+
+// E[mode][p1][perm(q)] = amp * exp(i * sum_n coef_n(mode) * w_k^n),  k = bin held by slot (p1, q),
+// perm(q) = (q & 15) << (logn2 - 4) | (q >> 4)  (the order k_rows reads).
+// coefs: device array [M][K] of dd, hh * beta_n / n!.  grid = (N / 256, M), block = 256.
+__global__ void k_etab(cpx* __restrict__ E, const dd* __restrict__ coefs, EtabParams P) {
+  const long long N = 1LL << (P.logn1 + P.logn2);
+  const long long slot = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (slot >= N) return;
+  const int mode = blockIdx.y;
+  const int p1 = (int)(slot >> P.logn2), q = (int)(slot & ((1LL << P.logn2) - 1));
+  const long long k = (long long)slot_to_bin_rt(P.logn1, p1) + ((long long)slot_to_bin_rt(P.logn2, q) << P.logn1);
+  const long long ks = (k < N / 2) ? k : k - N;  // Nyquist bin takes the negative frequency
+  const dd w = dd_mul_d(P.wstep, (double)ks);
+  const dd* c = coefs + (long long)mode * P.K;
+  dd ph = c[P.K - 1];
+  for (int n = P.K - 2; n >= 0; --n) ph = dd_add(dd_mul(ph, w), c[n]);
+  // reduce modulo 2 pi in double-double, then first-order correction for the low word
+  const double nrev = rint(ph.hi / P.twopi.hi);
+  dd r = dd_add(ph, dd_mul_d(P.twopi, -nrev));
+  double sn, cs;
+  sincos(r.hi, &sn, &cs);
+  const double sr = fma(cs, r.lo, sn), cr = fma(-sn, r.lo, cs);
+  const int qp = ((q & 15) << (P.logn2 - 4)) | (q >> 4);
+  E[(long long)mode * N + ((long long)p1 << P.logn2) + qp] = make_double2(P.amp * cr, P.amp * sr);
+}
+
+// slot -> bin map for the debug entry point.  grid = N/256
+__global__ void k_slot_map(long long* __restrict__ idx, int logn1, int logn2) {
+  const long long N = 1LL << (logn1 + logn2);
+  const long long slot = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (slot >= N) return;
+  const int p1 = (int)(slot >> logn2), q = (int)(slot & ((1LL << logn2) - 1));
+  idx[slot] = (long long)slot_to_bin_rt(logn1, p1) + ((long long)slot_to_bin_rt(logn2, q) << logn1);
+}
+
+// SPEC[r][bin(slot)] = X[r][slot]   (debug: natural-order spectrum).  grid = (N/256, 2M)
+__global__ void k_unpermute(const cpx* __restrict__ X, cpx* __restrict__ SPEC, int logn1, int logn2) {
+  const long long N = 1LL << (logn1 + logn2);
+  const long long slot = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (slot >= N) return;
+  const int p1 = (int)(slot >> logn2), q = (int)(slot & ((1LL << logn2) - 1));
+  const long long k = (long long)slot_to_bin_rt(logn1, p1) + ((long long)slot_to_bin_rt(logn2, q) << logn1);
+  SPEC[(long long)blockIdx.y * N + k] = X[(long long)blockIdx.y * N + slot];
+}
+
+}  // namespace mmf

@@ -7,8 +7,9 @@
 #include <vector>
 
 #include "../../include/mmf.h"
-#include "kernels.cuh"
+#include "fft_kernels.cuh"
 #include "nl_mma.cuh"
+#include "nl_simt.cuh"
 
 using namespace mmf;
 
@@ -26,8 +27,7 @@ int cuda_fail(cudaError_t e) {
     if (e__ != cudaSuccess) return cuda_fail(e__); \
   } while (0)
 
-constexpr int cols_logw(int logn1) { return logn1 <= 8 ? 4 : logn1 == 9 ? 3 : logn1 <= 11 ? 2 : 1; }
-constexpr int rows_logb(int logn2) { return logn2 >= 9 ? 0 : 9 - logn2; }
+constexpr int kGroups = 2;  // independent 256-thread groups per persistent transform CTA
 
 // exp(2 pi i p / n) for 0 <= p < n (n a power of two), long double with the angle folded to [0, pi/4] first,
 // so that the table is exactly symmetric and quarter turns are exact.  (Written independently of the oracle.)
@@ -84,6 +84,30 @@ int upload_roots(cpx** dptr, long long count, long long step, long long n) {
   return MMF_OK;
 }
 
+// stage twiddle tables of a 2^logp-point transform in the order fft_core.cuh reads them: stages most significant
+// digit first, stage (lr, logm) holding exp(2 pi i b c / 2^(lr+logm)) at [(c-1) << logm | b].
+int upload_stage_tables(cpx** dptr, int logp) {
+  std::vector<cpx> h;
+  int remain = logp, nst = nstages(logp);
+  while (nst > 0) {
+    const int lr = stage_lr(remain, nst), logm = remain - lr;
+    if (logm > 0)
+      for (int c = 1; c < (1 << lr); ++c)
+        for (int b = 0; b < (1 << logm); ++b) {
+          cpx w;
+          root_of_unity((long long)b * c, 1LL << (lr + logm), &w.x, &w.y);
+          h.push_back(w);
+        }
+    remain = logm;
+    --nst;
+  }
+  if ((int)h.size() != tw_total_entries(logp, nstages(logp))) return MMF_EINVAL;
+  if (h.empty()) h.push_back(make_double2(1.0, 0.0));
+  CU(cudaMalloc((void**)dptr, sizeof(cpx) * h.size()));
+  CU(cudaMemcpy(*dptr, h.data(), sizeof(cpx) * h.size(), cudaMemcpyHostToDevice));
+  return MMF_OK;
+}
+
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 }  // namespace
@@ -96,7 +120,7 @@ struct mmf_plan {
   double dt = 0, h = 0, alpha = 0, gamma = 0;
   std::vector<double> beta, kappa;
   double* d_kappa = nullptr;
-  cpx *d_tw1 = nullptr, *d_tw2 = nullptr, *d_whi = nullptr, *d_wlo = nullptr;
+  cpx *d_tw1 = nullptr, *d_tw2 = nullptr, *d_whi = nullptr, *d_wlo = nullptr, *d_colA = nullptr, *d_colB = nullptr;
   dd* d_coefs = nullptr;
   unsigned char* ws = nullptr;
   size_t ws_bytes = 0, field_bytes = 0;
@@ -145,19 +169,23 @@ void clear_events(mmf_plan* p) {
 // ---- launch helpers ----------------------------------------------------------------------------------------------
 template <int LOGN1, int DIR>
 int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
-  constexpr int LOGW = cols_logw(LOGN1);
-  constexpr int LOGTOT = LOGN1 + LOGW;
-  constexpr size_t smem = sizeof(cpx) << LOGTOT;
-  auto kern = k_cols<LOGN1, LOGW, DIR>;
+  constexpr int TWN = tw_total_entries(LOGN1, nstages(LOGN1));
+  constexpr size_t smem = sizeof(cpx) * (((TWN + 7) & ~7) + ((size_t)kGroups << MMF_TILE_LOG));
+  auto kern = k_cols<LOGN1, DIR, kGroups>;
   static bool attr_done = false;
   if (!attr_done) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_done = true;
   }
-  dim3 grid((unsigned)(1u << (p->logn2 - LOGW)), (unsigned)(2 * p->M), (unsigned)nbuf);
-  TwoLevelTw tw{p->d_whi, p->d_wlo, p->lb};
+  ColsParams q;
+  q.X0 = X0; q.X1 = X1;
+  q.twtab = p->d_tw1; q.whi = p->d_whi; q.wlo = p->d_wlo; q.colA = p->d_colA; q.colB = p->d_colB;
+  q.lb = p->lb; q.logn2 = p->logn2; q.nrows = 2 * p->M; q.nbuf = nbuf;
+  const long long tiles = ((long long)nbuf * 2 * p->M) << (p->logn2 - (MMF_TILE_LOG - LOGN1));
+  long long grid = (tiles + kGroups - 1) / kGroups;
+  if (grid > p->num_sms) grid = p->num_sms;
   LaunchTimer lt(p, DIR == 0 ? KC_COLS_FWD : KC_COLS_INV, st);
-  kern<<<grid, 1 << (LOGTOT - 4), smem, st>>>(X0, X1, p->d_tw1, tw, p->logn2);
+  kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(q);
   p->launches++;
   CU(cudaGetLastError());
   return MMF_OK;
@@ -167,31 +195,33 @@ template <int DIR>
 int launch_cols(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   switch (p->logn1) {
     case 6: return launch_cols_t<6, DIR>(p, X0, X1, nbuf, st);
-    case 7: return launch_cols_t<7, DIR>(p, X0, X1, nbuf, st);
     case 8: return launch_cols_t<8, DIR>(p, X0, X1, nbuf, st);
-    case 9: return launch_cols_t<9, DIR>(p, X0, X1, nbuf, st);
     case 10: return launch_cols_t<10, DIR>(p, X0, X1, nbuf, st);
-    case 11: return launch_cols_t<11, DIR>(p, X0, X1, nbuf, st);
     case 12: return launch_cols_t<12, DIR>(p, X0, X1, nbuf, st);
     default: return MMF_EINVAL;
   }
 }
 
-template <int LOGN2, int MODE>
+template <int LOGN2, int MODE, bool SINGLE>
 int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
-  constexpr int LOGB = rows_logb(LOGN2);
-  constexpr int LOGTOT = LOGN2 + LOGB;
-  constexpr size_t smem = sizeof(cpx) << LOGTOT;
-  auto kern = k_rows<LOGN2, LOGB, MODE>;
+  constexpr int TWN = tw_total_entries(LOGN2, nstages(LOGN2));
+  constexpr size_t smem = sizeof(cpx) * (((TWN + 7) & ~7) + ((size_t)kGroups << MMF_TILE_LOG));
+  constexpr int LOGB = MMF_TILE_LOG - LOGN2;
+  auto kern = k_rows<LOGN2, MODE, SINGLE, kGroups>;
   static bool attr_done = false;
   if (!attr_done) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_done = true;
   }
-  const long long nchunks = (2LL * p->M) << p->logn1;
-  dim3 grid((unsigned)((nchunks + (1 << LOGB) - 1) >> LOGB), 1, (unsigned)nbuf);
+  RowsParams q;
+  q.X0 = X0; q.X1 = X1; q.E = p->E; q.twtab = p->d_tw2;
+  q.nchunks = (2LL * p->M) << p->logn1;
+  q.logn1 = p->logn1; q.nbuf = nbuf; q.M = p->M;
+  const long long items = SINGLE ? ((q.nchunks + (1 << LOGB) - 1) >> LOGB) : ((long long)p->M << (p->logn1 - LOGB));
+  long long grid = (items + kGroups - 1) / kGroups;
+  if (grid > p->num_sms) grid = p->num_sms;
   LaunchTimer lt(p, KC_ROWS, st);
-  kern<<<grid, 1 << (LOGTOT - 4), smem, st>>>(X0, X1, p->E, p->d_tw2, nchunks, p->logn1);
+  kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(q);
   p->launches++;
   CU(cudaGetLastError());
   return MMF_OK;
@@ -199,16 +229,20 @@ int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
 
 template <int MODE>
 int launch_rows(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
+  if (p->logn1 == 0) {
+    switch (p->logn2) {
+#define MMF_ROWS_CASE(L) case L: return launch_rows_t<L, MODE, true>(p, X0, X1, nbuf, st);
+      MMF_ROWS_CASE(4) MMF_ROWS_CASE(5) MMF_ROWS_CASE(6) MMF_ROWS_CASE(7) MMF_ROWS_CASE(8) MMF_ROWS_CASE(9)
+      MMF_ROWS_CASE(10) MMF_ROWS_CASE(11) MMF_ROWS_CASE(12)
+#undef MMF_ROWS_CASE
+      default: return MMF_EINVAL;
+    }
+  }
   switch (p->logn2) {
-    case 4: return launch_rows_t<4, MODE>(p, X0, X1, nbuf, st);
-    case 5: return launch_rows_t<5, MODE>(p, X0, X1, nbuf, st);
-    case 6: return launch_rows_t<6, MODE>(p, X0, X1, nbuf, st);
-    case 7: return launch_rows_t<7, MODE>(p, X0, X1, nbuf, st);
-    case 8: return launch_rows_t<8, MODE>(p, X0, X1, nbuf, st);
-    case 9: return launch_rows_t<9, MODE>(p, X0, X1, nbuf, st);
-    case 10: return launch_rows_t<10, MODE>(p, X0, X1, nbuf, st);
-    case 11: return launch_rows_t<11, MODE>(p, X0, X1, nbuf, st);
-    case 12: return launch_rows_t<12, MODE>(p, X0, X1, nbuf, st);
+#define MMF_ROWS_CASE(L) case L: return launch_rows_t<L, MODE, false>(p, X0, X1, nbuf, st);
+    MMF_ROWS_CASE(6) MMF_ROWS_CASE(7) MMF_ROWS_CASE(8) MMF_ROWS_CASE(9) MMF_ROWS_CASE(10) MMF_ROWS_CASE(11)
+    MMF_ROWS_CASE(12)
+#undef MMF_ROWS_CASE
     default: return MMF_EINVAL;
   }
 }
@@ -317,6 +351,8 @@ void free_tables(mmf_plan* p) {
   cudaFree(p->d_tw2);
   cudaFree(p->d_whi);
   cudaFree(p->d_wlo);
+  cudaFree(p->d_colA);
+  cudaFree(p->d_colB);
   cudaFree(p->d_coefs);
 }
 
@@ -354,13 +390,13 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
   int logn = 0;
   while ((1LL << logn) < N) ++logn;
   p->logn = logn;
-  if (logn <= 12) {
-    p->logn1 = 0;
-    p->logn2 = logn;
-  } else {
-    p->logn2 = (logn + 1) / 2;
-    p->logn1 = logn - p->logn2;
-  }
+  // N = N1 N2: pass B (the FP64- and L1-heaviest pass: two transforms) gets the shorter transform where possible
+  if (logn <= MMF_TILE_LOG) p->logn1 = 0;
+  else if (logn == 13) p->logn1 = 6;
+  else if (logn <= 15) p->logn1 = 8;
+  else if (logn <= 22) p->logn1 = 10;
+  else p->logn1 = 12;
+  p->logn2 = logn - p->logn1;
   p->lb = (logn + 1) / 2;
   p->nlm_nk = (M <= MMF_NLM_MAXM) ? nlm_pick_nk(M) : -1;
   {
@@ -376,11 +412,18 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
     if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MMF_ENOMEM : cuda_fail(e); break; }
     e = cudaMemcpy(p->d_kappa, kappa, sizeof(double) * (size_t)M * M, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { rc = cuda_fail(e); break; }
-    if ((rc = upload_roots(&p->d_tw2, 1LL << p->logn2, 1, 1LL << p->logn2)) != MMF_OK) break;
+    if ((rc = upload_stage_tables(&p->d_tw2, p->logn2)) != MMF_OK) break;
     if (p->logn1 > 0) {
-      if ((rc = upload_roots(&p->d_tw1, 1LL << p->logn1, 1, 1LL << p->logn1)) != MMF_OK) break;
+      if ((rc = upload_stage_tables(&p->d_tw1, p->logn1)) != MMF_OK) break;
       if ((rc = upload_roots(&p->d_wlo, 1LL << p->lb, 1, N)) != MMF_OK) break;
       if ((rc = upload_roots(&p->d_whi, 1LL << (logn - p->lb), 1LL << p->lb, N)) != MMF_OK) break;
+      // steps of the inter-pass twiddle along the registers of the last pass-A stage (fft_kernels.cuh)
+      const int nst1 = nstages(p->logn1), lrl = last_lr(p->logn1, nst1), lrp = prev_lr(p->logn1, nst1);
+      const long long wA = 1LL << (p->logn1 - lrl);
+      const long long wB = (lrl == 4) ? 8 * wA : 1LL << (p->logn1 - lrl - lrp);
+      if (lrl < 3 || lrl > 4) { rc = MMF_EINVAL; break; }
+      if ((rc = upload_roots(&p->d_colA, 1LL << p->logn2, wA, N)) != MMF_OK) break;
+      if ((rc = upload_roots(&p->d_colB, 1LL << p->logn2, wB, N)) != MMF_OK) break;
     }
     // per-mode phase coefficients hh * beta_n / n! in double-double (hh = h/2, Eq. 6a)
     std::vector<dd> coefs((size_t)M * K);
