@@ -8,7 +8,7 @@
 
 #include "../../include/mmf.h"
 #include "fft_kernels.cuh"
-#include "nl_mma.cuh"
+#include "nl_tma.cuh"
 #include "nl_simt.cuh"
 
 using namespace mmf;
@@ -291,45 +291,81 @@ int nlm_pick_nk(int M) {
   return -1;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point query (no link-time dependency on libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)ptr;
+  }
+  return fn;
+}
+
+// tensor map of a field buffer [2M][N] complex128 seen as doubles [2M][2N], box = (8 samples = 16 doubles) x 2M rows
+int field_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) {
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled is unavailable");
+    return MMF_ECUDA;
+  }
+  const cuuint64_t gdim[2] = {(cuuint64_t)(2 * p->N), (cuuint64_t)(2 * p->M)};
+  const cuuint64_t gstride[1] = {(cuuint64_t)p->N * sizeof(cpx)};
+  const cuuint32_t box[2] = {2 * MMF_NLM_T, (cuuint32_t)(2 * p->M)};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return MMF_ECUDA;
+  }
+  return MMF_OK;
+}
+
+// PLAIN: A = U, B = OUT; other modes: A = X, B = Y.
 template <int NK, int MODE>
-int launch_nlm_t(mmf_plan* p, const cpx* U, cpx* X, cpx* Y, cudaStream_t st) {
-  auto kern = k_nlm<NK, MODE>;
+int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st) {
+  auto kern = k_nlt<NK, MODE>;
   constexpr int NARR = nlm_narr<MODE>();
-  NlmParams q;
-  q.U = U; q.X = X; q.Y = Y;
+  NltParams q;
   q.kappa = p->d_kappa;
   q.hg = p->h * p->gamma;
   q.M = p->M;
   q.NW = (p->M + 7) / 8;
-  q.N = p->N;
   q.ntiles = p->N / MMF_NLM_T;
-  const size_t gsm = nlm_group_smem(p->M, NK, NARR);
-  int tg = 16 / q.NW;                                  // at most 16 warps per CTA (128 registers per thread)
-  const int tg_smem = (int)((size_t)(200 * 1024) / gsm);
-  if (tg > tg_smem) tg = tg_smem;
-  while (tg > 1 && 32 * q.NW * tg > nlm_max_threads(NK)) --tg;   // the kernel's __launch_bounds__
-  if (tg < 1) return MMF_EINVAL;
-  if ((long long)tg > q.ntiles) tg = (int)q.ntiles;
-  q.TG = tg;
-  const size_t smem = gsm * tg;
+  CUtensorMap mapA, mapB;
+  int rc;
+  if ((rc = field_tile_map(p, A, &mapA)) != MMF_OK) return rc;
+  if ((rc = field_tile_map(p, B, &mapB)) != MMF_OK) return rc;
+  const size_t smem = nlt_smem_bytes(p->M, NK, NARR);
+  const int threads = 32 * (q.NW + 1);
   static size_t attr_smem = 0;
   if (smem > attr_smem) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_smem = smem;
   }
-  long long grid = (q.ntiles + tg - 1) / tg;
-  if (grid > p->num_sms) grid = p->num_sms;            // persistent: one CTA per SM
+  int occ = 1;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
+  if (occ < 1) return MMF_EINVAL;
+  long long grid = (long long)p->num_sms * occ;        // persistent: every resident CTA walks its own tile list
+  if (grid > q.ntiles) grid = q.ntiles;
   LaunchTimer lt(p, KC_NLM_PLAIN + MODE, st);
-  kern<<<(unsigned)grid, 32 * q.NW * tg, smem, st>>>(q);
+  kern<<<(unsigned)grid, threads, smem, st>>>(mapA, mapB, q);
   p->launches++;
   CU(cudaGetLastError());
   return MMF_OK;
 }
 
 template <int MODE>
-int launch_nlm(mmf_plan* p, const cpx* U, cpx* X, cpx* Y, cudaStream_t st) {
+int launch_nlm(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st) {
   switch (p->nlm_nk) {
-#define MMF_NLM_CASE(NKV) case NKV: return launch_nlm_t<NKV, MODE>(p, U, X, Y, st);
+#define MMF_NLM_CASE(NKV) case NKV: return launch_nlm_t<NKV, MODE>(p, A, B, st);
     MMF_NLM_CASE(1) MMF_NLM_CASE(2) MMF_NLM_CASE(3) MMF_NLM_CASE(4) MMF_NLM_CASE(6) MMF_NLM_CASE(8) MMF_NLM_CASE(9)
     MMF_NLM_CASE(12) MMF_NLM_CASE(16) MMF_NLM_CASE(20) MMF_NLM_CASE(24) MMF_NLM_CASE(28) MMF_NLM_CASE(30)
     MMF_NLM_CASE(32)
@@ -496,13 +532,13 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   int rc;
   if (p->nlm_nk > 0) {
     // two full-field buffers: X (the caller's field) and Y.  Per step: D(X,Y); S23 in place; D(X,Y); FINAL(+NEXT).
-    if ((rc = launch_nlm<NLM_PLAIN>(p, X, Y, nullptr, st)) != MMF_OK) return rc;   // Y <- h N(A) A   (6b bracket)
+    if ((rc = launch_nlm<NLM_PLAIN>(p, X, Y, st)) != MMF_OK) return rc;   // Y <- h N(A) A   (6b bracket)
     for (int s = 0; s < nsteps; ++s) {
       if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6a) A_I, (6b) k1
-      if ((rc = launch_nlm<NLM_S23>(p, nullptr, X, Y, st)) != MMF_OK) return rc;    // (6c), (6d), brackets of 6e/6f
+      if ((rc = launch_nlm<NLM_S23>(p, X, Y, st)) != MMF_OK) return rc;    // (6c), (6d), brackets of 6e/6f
       if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6e) argument, (6f) first term
-      if (s + 1 < nsteps) rc = launch_nlm<NLM_FINAL_NEXT>(p, nullptr, X, Y, st);    // (6e)+(6f), next (6b) bracket
-      else rc = launch_nlm<NLM_FINAL>(p, nullptr, X, Y, st);
+      if (s + 1 < nsteps) rc = launch_nlm<NLM_FINAL_NEXT>(p, X, Y, st);    // (6e)+(6f), next (6b) bracket
+      else rc = launch_nlm<NLM_FINAL>(p, X, Y, st);
       if (rc != MMF_OK) return rc;
     }
     return MMF_OK;
@@ -539,7 +575,7 @@ int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
 
 int mmf_apply_nonlinear(mmf_plan* p, const void* U_dev, void* OUT_dev, void* cuda_stream) {
   if (!p || !U_dev || !OUT_dev || (((size_t)U_dev | (size_t)OUT_dev) & 15) != 0) return MMF_EINVAL;
-  if (p->nlm_nk > 0) return launch_nlm<NLM_PLAIN>(p, (const cpx*)U_dev, (cpx*)OUT_dev, nullptr, (cudaStream_t)cuda_stream);
+  if (p->nlm_nk > 0) return launch_nlm<NLM_PLAIN>(p, (const cpx*)U_dev, (cpx*)OUT_dev, (cudaStream_t)cuda_stream);
   return launch_nl<NL_PLAIN>(p, (cpx*)U_dev, (cpx*)OUT_dev, nullptr, nullptr, (cudaStream_t)cuda_stream);
 }
 
