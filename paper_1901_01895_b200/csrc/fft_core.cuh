@@ -203,30 +203,34 @@ __device__ __forceinline__ void stage_math(cpx (&v)[16], int base, const cpx* __
 // concatenated tables of the LOGP-point transform, bar = the group's named-barrier id.
 // FENCE: also synchronise after the last exchange read (needed when the caller's next use of the buffer does not
 // start with the slots this thread read last, i.e. when the chain is not followed by its adjoint).
-template <int LOGTOT, int LOGP, int LOGW, int REMAIN, int NST, int SIGN, bool FENCE>
+// PRESYNC: also synchronise before the FIRST exchange write (needed when the caller took v from the exchange buffer
+// itself in a different layout — a tile staged there by TMA — so that nobody overwrites a value not yet read).
+template <int LOGTOT, int LOGP, int LOGW, int REMAIN, int NST, int SIGN, bool FENCE, bool PRESYNC = false>
 __device__ __forceinline__ void fft_dif(cpx (&v)[16], cpx* __restrict__ s, int t, const cpx* __restrict__ tab, int bar) {
   constexpr int LR = stage_lr(REMAIN, NST), LOGM = REMAIN - LR, LO = stage_lo(LOGM, LOGW, LOGTOT);
   const int base = stage_base<LO>(t);
   stage_math<LOGTOT, LOGW, LOGM, LR, SIGN, true>(v, base, tab + tw_offset(LOGP, REMAIN, NST));
   if constexpr (NST > 1) {
     constexpr int LR2 = stage_lr(LOGM, NST - 1), LO2 = stage_lo(LOGM - LR2, LOGW, LOGTOT);
+    if constexpr (PRESYNC && REMAIN == LOGP) group_barrier(bar, MMF_GROUP_THREADS);
     tile_sts<LO>(v, s, base);
     group_barrier(bar, MMF_GROUP_THREADS);
     tile_lds<LO2>(v, s, stage_base<LO2>(t));
     if constexpr (FENCE && NST == 2) group_barrier(bar, MMF_GROUP_THREADS);
-    fft_dif<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, FENCE>(v, s, t, tab, bar);
+    fft_dif<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, FENCE, PRESYNC>(v, s, t, tab, bar);
   }
 }
 
 // Inverse chain (DIT, least significant digit first): the adjoint of fft_dif with the opposite SIGN.  Entry: v in the
 // layout of the last stage; exit: v in the layout of stage (REMAIN, NST) of the outermost call, natural order.
-template <int LOGTOT, int LOGP, int LOGW, int REMAIN, int NST, int SIGN, bool FENCE>
+template <int LOGTOT, int LOGP, int LOGW, int REMAIN, int NST, int SIGN, bool FENCE, bool PRESYNC = false>
 __device__ __forceinline__ void fft_dit(cpx (&v)[16], cpx* __restrict__ s, int t, const cpx* __restrict__ tab, int bar) {
   constexpr int LR = stage_lr(REMAIN, NST), LOGM = REMAIN - LR, LO = stage_lo(LOGM, LOGW, LOGTOT);
   const int base = stage_base<LO>(t);
   if constexpr (NST > 1) {
     constexpr int LR2 = stage_lr(LOGM, NST - 1), LO2 = stage_lo(LOGM - LR2, LOGW, LOGTOT);
-    fft_dit<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, false>(v, s, t, tab, bar);
+    fft_dit<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, false, PRESYNC>(v, s, t, tab, bar);
+    if constexpr (PRESYNC && NST == 2) group_barrier(bar, MMF_GROUP_THREADS);
     tile_sts<LO2>(v, s, stage_base<LO2>(t));
     group_barrier(bar, MMF_GROUP_THREADS);
     tile_lds<LO>(v, s, base);

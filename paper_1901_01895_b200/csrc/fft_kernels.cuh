@@ -17,6 +17,7 @@
 // butterflies.  Global loads go straight into the registers of the first stage and the last stage stores from
 // registers.
 #pragma once
+#include "async_copy.cuh"
 #include "fft_core.cuh"
 
 namespace mmf {
@@ -46,26 +47,25 @@ __device__ __forceinline__ void load_stage_tables(cpx* __restrict__ tab, const c
 }
 
 // ---------------------------------------------------------------------------------------------------- pass A / C
+// Inter-pass table (filled by the host, mmf_api.cu): one row of 256 + 2 W entries per column tile ct,
+//   [t]           W_N^(k1(pos0(t)) n2(t)),  pos0(t) = 16 (t >> LOGW) the first slot thread t holds after the last
+//                 pass-A stage, n2(t) = ct W + (t & (W - 1)) its column;
+//   [256 + c]     W_N^(wA n2),  [256 + W + c]  W_N^(wB n2),  n2 = ct W + c: the steps of the exponent along the
+//                 16 registers of that layout, k1(pos0 + j) = k1(pos0) + wA (j & 7) + wB (j >> 3).
+// The row travels to shared memory with the tile (one bulk copy), so the kernel makes no global load of its own.
+__host__ __device__ constexpr int ipt_row_entries(int logw) { return 256 + (2 << logw); }
+
 struct ColsParams {
-  cpx* X0;
-  cpx* X1;
   const cpx* __restrict__ twtab;  // stage tables of the N1-point transform
-  const cpx* __restrict__ whi;    // W_N^x = whi[x >> lb] * wlo[x & (2^lb - 1)]
-  const cpx* __restrict__ wlo;
-  const cpx* __restrict__ colA;   // [N2]  W_N^(wA n2): step of register bit 0 of the last-stage layout
-  const cpx* __restrict__ colB;   // [N2]  W_N^(wB n2): step of register bit 3
-  int lb, logn2, nrows, nbuf;
+  const cpx* __restrict__ ipt;    // inter-pass table [N2 / W][256 + 2 W]
+  int logn2, nrows, nbuf;
 };
 
-// v[j] *= W_N^(k1(pos0 + j) n2)  (or its conjugate): k1(pos0 + j) = k1(pos0) + wA (j & 7) + wB (j >> 3), so the 16
-// factors are t0 sA^(j&7) sB^(j>>3) — three table look-ups per thread and short product chains (depth <= 4)
-// instead of 32 gathers.
-template <int LOGN1, bool CONJ>
-__device__ __forceinline__ void apply_interpass(cpx (&v)[16], int pos0, long long n2, const ColsParams& p) {
-  const long long x = (long long)slot_to_bin<LOGN1>(pos0) * n2;
-  const cpx t0 = cmul(p.whi[x >> p.lb], p.wlo[x & ((1LL << p.lb) - 1)]);
-  const cpx sA = p.colA[n2];
-  const cpx t1 = cmul(t0, p.colB[n2]);
+// v[j] *= W_N^(k1(pos0 + j) n2)  (or its conjugate): the 16 factors are t0 sA^(j&7) sB^(j>>3) — three look-ups per
+// thread and short product chains (depth <= 4).
+template <bool CONJ>
+__device__ __forceinline__ void apply_interpass(cpx (&v)[16], cpx t0, cpx sA, cpx sB) {
+  const cpx t1 = cmul(t0, sB);
   cpx pw[8];
   pw[1] = sA;
   pw[2] = cmul(sA, sA);
@@ -84,55 +84,156 @@ __device__ __forceinline__ void apply_interpass(cpx (&v)[16], int pos0, long lon
   }
 }
 
-// grid = persistent (<= one CTA per SM); block = 256 G.  DIR 0: pass A (DIF, sign +, then twiddle);
-// DIR 1: pass C (conjugate twiddle, then DIT, sign -).  A tile is N1 points x W = 2^(12 - LOGN1) adjacent columns.
-// dynamic shared memory: stage tables + G exchange buffers.
+// un-swizzled tile access: the layout TMA writes / reads (tile element f at slot f)
+template <int LO>
+__device__ __forceinline__ void tile_lds_linear(cpx (&v)[16], const cpx* __restrict__ s, int base) {
+#pragma unroll
+  for (int j = 0; j < 16; ++j) v[j] = s[base | (j << LO)];
+}
+template <int LO>
+__device__ __forceinline__ void tile_sts_linear(const cpx (&v)[16], cpx* __restrict__ s, int base) {
+#pragma unroll
+  for (int j = 0; j < 16; ++j) s[base | (j << LO)] = v[j];
+}
+
+// number of tile slots of the pass A / C ring: three where the stage tables leave room (N1 <= 2^10), else two
+__host__ __device__ constexpr int cols_slots(int logn1) { return logn1 <= 10 ? 3 : 2; }
+template <int LOGN1>
+__host__ __device__ constexpr size_t cols_smem_bytes() {
+  constexpr int TWN = tw_total_entries(LOGN1, nstages(LOGN1));
+  return sizeof(cpx) * (((size_t)cols_slots(LOGN1) << MMF_TILE_LOG) +
+                        (size_t)cols_slots(LOGN1) * ipt_row_entries(MMF_TILE_LOG - LOGN1) + ((TWN + 7) & ~7)) + 64;
+}
+
+// grid = persistent (<= one CTA per SM); block = 512 = two groups of 256.  DIR 0: pass A (DIF, sign +, then twiddle);
+// DIR 1: pass C (conjugate twiddle, then DIT, sign -).  A tile is N1 points x W = 2^(12 - LOGN1) adjacent columns of
+// one field row, i.e. the box (2 W doubles, N1 rows) of the 2-D tensor map (inner = 2 N2 doubles, outer = rows x N1,
+// stride N2 complex) at (2 W ct, row N1), moved in boxes of <= 256 rows.
+// Data movement is asynchronous and off the LSU pipe: the CTA's tiles t = 0, 1, 2, ... rotate through S ring slots
+// (slot t % S), tile t is worked on by group t % 2 IN its slot (the slot is also the group's exchange buffer), and the
+// group's first thread stores it with TMA and then refills the slot its previous tile vacated with tile t - 2 + S,
+// which the other group picks up half a tile period later.  map0 / map1: the two field buffers.
 template <int LOGN1, int DIR, int G>
-__global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_cols(ColsParams p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+__global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1)
+k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, ColsParams p) {
+  static_assert(G == 2, "two groups alternate over the ring");
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
   constexpr int LOGW = MMF_TILE_LOG - LOGN1, W = 1 << LOGW;
   constexpr int NST = nstages(LOGN1);
   constexpr int TWN = tw_total_entries(LOGN1, NST);
   constexpr int LR1 = stage_lr(LOGN1, NST), LO1 = stage_lo(LOGN1 - LR1, LOGW, MMF_TILE_LOG);  // first-stage layout
   constexpr int LOL = stage_lo(0, LOGW, MMF_TILE_LOG);                                        // last-stage layout
-  cpx* tab = reinterpret_cast<cpx*>(smem_raw);
-  load_stage_tables<TWN>(tab, p.twtab);
+  constexpr int S = cols_slots(LOGN1);
+  constexpr int TILE_BYTES = (int)sizeof(cpx) << MMF_TILE_LOG;
+  constexpr int RB = LOGN1 > 8 ? 256 : (1 << LOGN1);  // rows per TMA box
+  constexpr int NBOX = (1 << LOGN1) / RB;
+  constexpr int BOX_BYTES = RB * W * (int)sizeof(cpx);
+  constexpr int IPT = ipt_row_entries(LOGW);
+  static_assert(NST >= 2, "the ring protocol assumes at least one exchange");
+  cpx* ring = reinterpret_cast<cpx*>(smem_raw);
+  cpx* ipts = ring + ((size_t)S << MMF_TILE_LOG);
+  cpx* tab = ipts + S * IPT;
+  uint64_t* full = reinterpret_cast<uint64_t*>(tab + ((TWN + 7) & ~7));
+  uint64_t* done = full + S;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
+#pragma unroll
+    for (int i = 0; i < G; ++i) mbar_init(&done[i], MMF_GROUP_THREADS);
+    mbar_init_fence();
+    tma_prefetch_desc(&map0);
+    tma_prefetch_desc(&map1);
+  }
+  load_stage_tables<TWN>(tab, p.twtab);  // ends with __syncthreads
   const int grp = threadIdx.x / MMF_GROUP_THREADS, t = threadIdx.x % MMF_GROUP_THREADS;
-  cpx* s = tab + ((TWN + 7) & ~7) + (grp << MMF_TILE_LOG);
+  const bool elect = t == 0;
   const int bar = 1 + grp;
   const int logn2 = p.logn2;
-  const long long N = 1LL << (LOGN1 + logn2);
   const long long nct = 1LL << (logn2 - LOGW);
   const long long total = nct * p.nrows * p.nbuf;
+  const long long ntile = total > blockIdx.x ? (total - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+
+  // global coordinates of the CTA's tile tt, and its TMA traffic
+  auto tile_coords = [&](long long tt, int& c0, int& c1, const CUtensorMap*& m, long long& ct) {
+    const long long u = blockIdx.x + tt * gridDim.x;
+    ct = u & (nct - 1);
+    const long long rb = u >> (logn2 - LOGW);
+    c0 = (int)(ct << (LOGW + 1));                       // doubles
+    c1 = (int)(rb % p.nrows) << LOGN1;                  // memory row of the (rows x N1, N2) view
+    m = (rb / p.nrows) ? &map1 : &map0;
+  };
+  auto issue_load = [&](long long tt) {
+    int c0, c1;
+    const CUtensorMap* m;
+    long long ct;
+    tile_coords(tt, c0, c1, m, ct);
+    const int b = (int)(tt % S);
+    mbar_arrive_expect_tx(&full[b], TILE_BYTES + IPT * (int)sizeof(cpx));
+    unsigned char* dst = smem_raw + (size_t)b * TILE_BYTES;
+#pragma unroll
+    for (int i = 0; i < NBOX; ++i) tma_load_2d(dst + i * BOX_BYTES, m, c0, c1 + i * RB, &full[b]);
+    bulk_load_1d(ipts + b * IPT, p.ipt + ct * IPT, IPT * (int)sizeof(cpx), &full[b]);
+  };
+  auto issue_store = [&](long long tt) {
+    int c0, c1;
+    const CUtensorMap* m;
+    long long ct;
+    tile_coords(tt, c0, c1, m, ct);
+    const unsigned char* src = smem_raw + (size_t)(tt % S) * TILE_BYTES;
+#pragma unroll
+    for (int i = 0; i < NBOX; ++i) tma_store_2d(m, c0, c1 + i * RB, src + i * BOX_BYTES);
+    tma_store_commit();
+  };
+
+  if (threadIdx.x == 0)
+    for (long long tt = 0; tt < S && tt < ntile; ++tt) issue_load(tt);
+
   const int base1 = stage_base<LO1>(t), basel = stage_base<LOL>(t);
-  const int pos0 = basel >> LOGW, c = t & (W - 1);
-  for (long long u = (long long)blockIdx.x * G + grp; u < total; u += (long long)gridDim.x * G) {
-    const long long ct = u & (nct - 1), rb = u >> (logn2 - LOGW);
-    const int row = (int)(rb % p.nrows), buf = (int)(rb / p.nrows);
-    cpx* g = (buf ? p.X1 : p.X0) + (long long)row * N + (ct << LOGW);
+  const int c = t & (W - 1);
+  int it = 0;
+  for (long long tt = grp; tt < ntile; tt += G, ++it) {
+    const int b = (int)(tt % S);
+    cpx* s = ring + ((size_t)b << MMF_TILE_LOG);
+    const cpx* ip = ipts + b * IPT;
+    // the slot this group's previous tile (tt - 2) left: refill it with tile tt - 2 + S once its store has read it
+    const bool refill = elect && tt >= G && tt - G + S < ntile;
+    if (S == 2 && refill) {
+      tma_store_wait_read();
+      issue_load(tt - G + S);
+    }
+    mbar_wait(&full[b], (uint32_t)((tt / S) & 1));
     cpx v[16];
     if constexpr (DIR == 0) {
-#pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const int f = base1 | (j << LO1);
-        v[j] = ld_stream(g + (((long long)(f >> LOGW)) << logn2) + (f & (W - 1)));
+      tile_lds_linear<LO1>(v, s, base1);
+      if (S > 2 && refill) {
+        tma_store_wait_read();
+        issue_load(tt - G + S);
       }
-      fft_dif<MMF_TILE_LOG, LOGN1, LOGW, LOGN1, NST, +1, true>(v, s, t, tab, bar);
-      apply_interpass<LOGN1, false>(v, pos0, (ct << LOGW) + c, p);
-#pragma unroll
-      for (int j = 0; j < 16; ++j) st_stream(g + (((long long)(pos0 + j)) << logn2) + c, v[j]);
+      fft_dif<MMF_TILE_LOG, LOGN1, LOGW, LOGN1, NST, +1, false, true>(v, s, t, tab, bar);
+      apply_interpass<false>(v, ip[t], ip[256 + c], ip[256 + W + c]);
+      group_barrier(bar, MMF_GROUP_THREADS);  // everybody has read the last exchange
+      tile_sts_linear<LOL>(v, s, basel);
     } else {
-#pragma unroll
-      for (int j = 0; j < 16; ++j) v[j] = ld_stream(g + (((long long)(pos0 + j)) << logn2) + c);
-      apply_interpass<LOGN1, true>(v, pos0, (ct << LOGW) + c, p);
-      fft_dit<MMF_TILE_LOG, LOGN1, LOGW, LOGN1, NST, -1, true>(v, s, t, tab, bar);
-#pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const int f = base1 | (j << LO1);
-        st_stream(g + (((long long)(f >> LOGW)) << logn2) + (f & (W - 1)), v[j]);
+      tile_lds_linear<LOL>(v, s, basel);
+      const cpx t0 = ip[t], sA = ip[256 + c], sB = ip[256 + W + c];
+      if (S > 2 && refill) {
+        tma_store_wait_read();
+        issue_load(tt - G + S);
       }
+      apply_interpass<true>(v, t0, sA, sB);
+      fft_dit<MMF_TILE_LOG, LOGN1, LOGW, LOGN1, NST, -1, false, true>(v, s, t, tab, bar);
+      group_barrier(bar, MMF_GROUP_THREADS);
+      tile_sts_linear<LO1>(v, s, base1);
+    }
+    // hand the finished tile to the async proxy: every thread's writes are fenced, the first thread stores
+    fence_proxy_async_smem();
+    mbar_arrive(&done[grp]);
+    if (elect) {
+      mbar_wait(&done[grp], (uint32_t)(it & 1));
+      issue_store(tt);
     }
   }
+  if (elect) tma_store_wait_all();
 }
 
 // -------------------------------------------------------------------------------------------------------- pass B
@@ -155,7 +256,7 @@ struct RowsParams {
 // one piece of the table and are done back to back by the same group, so the table is read from HBM once.
 template <int LOGN2, int MODE, bool SINGLE, int G>
 __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
   constexpr int LOGB = MMF_TILE_LOG - LOGN2;
   constexpr int NST = nstages(LOGN2);
   constexpr int TWN = tw_total_entries(LOGN2, NST);

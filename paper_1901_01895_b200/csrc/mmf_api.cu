@@ -76,14 +76,6 @@ void root_of_unity(long long p, long long n, double* re, double* im) {
   *im = (double)ci;
 }
 
-int upload_roots(cpx** dptr, long long count, long long step, long long n) {
-  std::vector<cpx> h((size_t)count);
-  for (long long i = 0; i < count; ++i) root_of_unity(i * step, n, &h[i].x, &h[i].y);
-  CU(cudaMalloc((void**)dptr, sizeof(cpx) * (size_t)count));
-  CU(cudaMemcpy(*dptr, h.data(), sizeof(cpx) * (size_t)count, cudaMemcpyHostToDevice));
-  return MMF_OK;
-}
-
 // stage twiddle tables of a 2^logp-point transform in the order fft_core.cuh reads them: stages most significant
 // digit first, stage (lr, logm) holding exp(2 pi i b c / 2^(lr+logm)) at [(c-1) << logm | b].
 int upload_stage_tables(cpx** dptr, int logp) {
@@ -113,14 +105,14 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 }  // namespace
 
 struct mmf_plan {
-  int M = 0, K = 0, logn = 0, logn1 = 0, logn2 = 0, lb = 0;
+  int M = 0, K = 0, logn = 0, logn1 = 0, logn2 = 0;
   int nlm_nk = -1;   // k-steps of the tensor-path nonlinear kernel; -1: M too large, legacy kernels (4 buffers)
   int num_sms = 148;
   long long N = 0;
   double dt = 0, h = 0, alpha = 0, gamma = 0;
   std::vector<double> beta, kappa;
   double* d_kappa = nullptr;
-  cpx *d_tw1 = nullptr, *d_tw2 = nullptr, *d_whi = nullptr, *d_wlo = nullptr, *d_colA = nullptr, *d_colB = nullptr;
+  cpx *d_tw1 = nullptr, *d_tw2 = nullptr, *d_ipt = nullptr;
   dd* d_coefs = nullptr;
   unsigned char* ws = nullptr;
   size_t ws_bytes = 0, field_bytes = 0;
@@ -166,11 +158,50 @@ void clear_events(mmf_plan* p) {
   p->ev_class.clear();
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point query (no link-time dependency on libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)ptr;
+  }
+  return fn;
+}
+
+// tensor map of a field buffer for passes A / C: the buffer seen as doubles [2M N1][2 N2] (memory rows of N2 complex
+// values), box = (2 W doubles = W adjacent columns) x min(N1, 256) rows
+int cols_tile_map(const mmf_plan* p, const void* base, int logn1, CUtensorMap* map) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) {
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled is unavailable");
+    return MMF_ECUDA;
+  }
+  const int logw = MMF_TILE_LOG - logn1;
+  const cuuint64_t gdim[2] = {(cuuint64_t)2 << p->logn2, ((cuuint64_t)(2 * p->M)) << logn1};
+  const cuuint64_t gstride[1] = {sizeof(cpx) << p->logn2};
+  const cuuint32_t box[2] = {(cuuint32_t)2 << logw, (cuuint32_t)(logn1 > 8 ? 256 : (1 << logn1))};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return MMF_ECUDA;
+  }
+  return MMF_OK;
+}
+
 // ---- launch helpers ----------------------------------------------------------------------------------------------
 template <int LOGN1, int DIR>
 int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
-  constexpr int TWN = tw_total_entries(LOGN1, nstages(LOGN1));
-  constexpr size_t smem = sizeof(cpx) * (((TWN + 7) & ~7) + ((size_t)kGroups << MMF_TILE_LOG));
+  constexpr size_t smem = cols_smem_bytes<LOGN1>();
+  constexpr int LOGW = MMF_TILE_LOG - LOGN1;
   auto kern = k_cols<LOGN1, DIR, kGroups>;
   static bool attr_done = false;
   if (!attr_done) {
@@ -178,14 +209,16 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
     attr_done = true;
   }
   ColsParams q;
-  q.X0 = X0; q.X1 = X1;
-  q.twtab = p->d_tw1; q.whi = p->d_whi; q.wlo = p->d_wlo; q.colA = p->d_colA; q.colB = p->d_colB;
-  q.lb = p->lb; q.logn2 = p->logn2; q.nrows = 2 * p->M; q.nbuf = nbuf;
-  const long long tiles = ((long long)nbuf * 2 * p->M) << (p->logn2 - (MMF_TILE_LOG - LOGN1));
-  long long grid = (tiles + kGroups - 1) / kGroups;
-  if (grid > p->num_sms) grid = p->num_sms;
+  q.twtab = p->d_tw1; q.ipt = p->d_ipt;
+  q.logn2 = p->logn2; q.nrows = 2 * p->M; q.nbuf = nbuf;
+  CUtensorMap map0, map1;
+  int rc;
+  if ((rc = cols_tile_map(p, X0, LOGN1, &map0)) != MMF_OK) return rc;
+  if ((rc = cols_tile_map(p, nbuf > 1 ? X1 : X0, LOGN1, &map1)) != MMF_OK) return rc;
+  const long long tiles = ((long long)nbuf * 2 * p->M) << (p->logn2 - LOGW);
+  long long grid = tiles < p->num_sms ? tiles : p->num_sms;
   LaunchTimer lt(p, DIR == 0 ? KC_COLS_FWD : KC_COLS_INV, st);
-  kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(q);
+  kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(map0, map1, q);
   p->launches++;
   CU(cudaGetLastError());
   return MMF_OK;
@@ -291,22 +324,6 @@ int nlm_pick_nk(int M) {
   return -1;
 }
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point query (no link-time dependency on libcuda)
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-EncodeTiledFn encode_tiled_fn() {
-  static EncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void* ptr = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-      fn = (EncodeTiledFn)ptr;
-  }
-  return fn;
-}
-
 // tensor map of a field buffer [2M][N] complex128 seen as doubles [2M][2N], box = (8 samples = 16 doubles) x 2M rows
 int field_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
   EncodeTiledFn enc = encode_tiled_fn();
@@ -385,10 +402,7 @@ void free_tables(mmf_plan* p) {
   cudaFree(p->d_kappa);
   cudaFree(p->d_tw1);
   cudaFree(p->d_tw2);
-  cudaFree(p->d_whi);
-  cudaFree(p->d_wlo);
-  cudaFree(p->d_colA);
-  cudaFree(p->d_colB);
+  cudaFree(p->d_ipt);
   cudaFree(p->d_coefs);
 }
 
@@ -433,7 +447,6 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
   else if (logn <= 22) p->logn1 = 10;
   else p->logn1 = 12;
   p->logn2 = logn - p->logn1;
-  p->lb = (logn + 1) / 2;
   p->nlm_nk = (M <= MMF_NLM_MAXM) ? nlm_pick_nk(M) : -1;
   {
     int dev = 0, sms = 0;
@@ -451,15 +464,30 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
     if ((rc = upload_stage_tables(&p->d_tw2, p->logn2)) != MMF_OK) break;
     if (p->logn1 > 0) {
       if ((rc = upload_stage_tables(&p->d_tw1, p->logn1)) != MMF_OK) break;
-      if ((rc = upload_roots(&p->d_wlo, 1LL << p->lb, 1, N)) != MMF_OK) break;
-      if ((rc = upload_roots(&p->d_whi, 1LL << (logn - p->lb), 1LL << p->lb, N)) != MMF_OK) break;
-      // steps of the inter-pass twiddle along the registers of the last pass-A stage (fft_kernels.cuh)
+      // inter-pass table (fft_kernels.cuh): per column tile, W_N^(k1(pos0(t)) n2(t)) for the 256 threads of a group
+      // and the steps W_N^(wA n2), W_N^(wB n2) of the exponent along the registers of the last pass-A stage
       const int nst1 = nstages(p->logn1), lrl = last_lr(p->logn1, nst1), lrp = prev_lr(p->logn1, nst1);
       const long long wA = 1LL << (p->logn1 - lrl);
       const long long wB = (lrl == 4) ? 8 * wA : 1LL << (p->logn1 - lrl - lrp);
       if (lrl < 3 || lrl > 4) { rc = MMF_EINVAL; break; }
-      if ((rc = upload_roots(&p->d_colA, 1LL << p->logn2, wA, N)) != MMF_OK) break;
-      if ((rc = upload_roots(&p->d_colB, 1LL << p->logn2, wB, N)) != MMF_OK) break;
+      const int logw = MMF_TILE_LOG - p->logn1, W = 1 << logw, ipt = ipt_row_entries(logw);
+      const long long nct = 1LL << (p->logn2 - logw);
+      std::vector<cpx> h((size_t)nct * ipt);
+      for (long long ct = 0; ct < nct; ++ct) {
+        cpx* row = h.data() + (size_t)ct * ipt;
+        for (int t = 0; t < 256; ++t) {
+          const long long k1 = slot_to_bin_rt(p->logn1, 16 * (t >> logw)), n2 = ct * W + (t & (W - 1));
+          root_of_unity(k1 * n2, N, &row[t].x, &row[t].y);
+        }
+        for (int c = 0; c < W; ++c) {
+          root_of_unity(wA * (ct * W + c), N, &row[256 + c].x, &row[256 + c].y);
+          root_of_unity(wB * (ct * W + c), N, &row[256 + W + c].x, &row[256 + W + c].y);
+        }
+      }
+      cudaError_t e2 = cudaMalloc((void**)&p->d_ipt, sizeof(cpx) * h.size());
+      if (e2 != cudaSuccess) { rc = (e2 == cudaErrorMemoryAllocation) ? MMF_ENOMEM : cuda_fail(e2); break; }
+      e2 = cudaMemcpy(p->d_ipt, h.data(), sizeof(cpx) * h.size(), cudaMemcpyHostToDevice);
+      if (e2 != cudaSuccess) { rc = cuda_fail(e2); break; }
     }
     // per-mode phase coefficients hh * beta_n / n! in double-double (hh = h/2, Eq. 6a)
     std::vector<dd> coefs((size_t)M * K);

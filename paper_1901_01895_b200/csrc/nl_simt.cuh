@@ -48,7 +48,7 @@ __device__ __forceinline__ cpx nl_arg(const NlParams& p, long long i) {
 // dynamic shared memory: 2 * M * 32 doubles.
 template <int MODE>
 __global__ void __launch_bounds__(MMF_NL_T* MMF_NL_WARPS) k_nl(NlParams p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* P1 = reinterpret_cast<double*>(smem_raw);
   double* P2 = P1 + (size_t)p.M * MMF_NL_T;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;

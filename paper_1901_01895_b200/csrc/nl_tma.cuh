@@ -80,7 +80,7 @@ __device__ __forceinline__ cpx axpy(double s, cpx a, cpx b) { return make_double
 template <int NK, int MODE>
 __global__ void __launch_bounds__(512, 1)
 k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, NltParams p) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
   constexpr int NARR = nlm_narr<MODE>();
   constexpr bool TWO_ROUNDS = (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;

@@ -85,7 +85,8 @@ def test_forward_transform_integer_exact(mmf, torch, orc, logn):
 
 
 # ------------------------------------------------------------------------------------------------ linear operator D
-@pytest.mark.parametrize("cfg,M,logn", [(0, 2, 12), (1, 3, 13), (1, 2, 16), (2, 3, 14), (3, 5, 18), (4, 2, 15), (4, 1, 4)])
+@pytest.mark.parametrize("cfg,M,logn", [(0, 2, 12), (1, 3, 13), (1, 2, 16), (2, 3, 14), (3, 5, 18), (4, 2, 15), (4, 1, 4),
+                                        (4, 1, 22), (4, 1, 23)])
 def test_linear_operator_matches_oracle(mmf, torch, orc, cfg, M, logn):
     p = workloads.problem(cfg, M=M, N=1 << logn)
     A = p.field()
