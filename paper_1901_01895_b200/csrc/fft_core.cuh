@@ -126,7 +126,13 @@ __host__ __device__ __forceinline__ constexpr int slot_to_bin(int p) {
 // butterfly at low index b by exp(+-2 pi i b c / 2^(LR+LOGM)).  Table of one stage: entry [(c-1) << LOGM | b],
 // c = 1 .. 2^LR - 1, b < 2^LOGM (stages with LOGM = 0 have none).  Tables of all stages are concatenated, most
 // significant digit first.  (The host fills them with the same recursion, mmf_api.cu.)
-__host__ __device__ constexpr int tw_stage_entries(int lr, int logm) { return logm > 0 ? (((1 << lr) - 1) << logm) : 0; }
+// COMPACT stages (radix 16 over 256 points below, the one big table: 61 KB): only c = 1, 2, 3 (rows 0-2) and
+// c = 4, 8, 12 (rows 3-5) are stored and w^(b (4 c1 + c0)) = w^(4 b c1) w^(b c0) costs one more product for the nine
+// mixed entries — 24 KB instead of 61 KB of shared memory, and 6 instead of 15 table reads per thread.
+__host__ __device__ constexpr bool tw_compact(int lr, int logm) { return lr == 4 && logm == 8; }
+__host__ __device__ constexpr int tw_stage_entries(int lr, int logm) {
+  return logm > 0 ? ((tw_compact(lr, logm) ? 6 : ((1 << lr) - 1)) << logm) : 0;
+}
 __host__ __device__ constexpr int tw_total_entries(int remain, int nst) {
   return nst <= 0 ? 0
                   : tw_stage_entries(stage_lr(remain, nst), remain - stage_lr(remain, nst)) +
@@ -162,6 +168,28 @@ __device__ __forceinline__ void group_barrier(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
 }
 
+// x[c] *= w^(SIGN b c), c = 1 .. R-1, from this stage's table (full: row c-1; compact: see tw_compact)
+template <int R, int LR, int LOGM, int SIGN>
+__device__ __forceinline__ void stage_twiddle(cpx (&x)[R], const cpx* __restrict__ tab, int b) {
+  if constexpr (tw_compact(LR, LOGM)) {
+    cpx lo[4], hi[4];
+#pragma unroll
+    for (int i = 1; i < 4; ++i) {
+      lo[i] = tab[((i - 1) << LOGM) | b];
+      hi[i] = tab[((i + 2) << LOGM) | b];
+    }
+#pragma unroll
+    for (int c = 1; c < R; ++c) {
+      const int c0 = c & 3, c1 = c >> 2;
+      const cpx w = c1 == 0 ? lo[c0] : c0 == 0 ? hi[c1] : cmul(hi[c1], lo[c0]);
+      x[c] = cmul_s<SIGN>(x[c], w);
+    }
+  } else {
+#pragma unroll
+    for (int c = 1; c < R; ++c) x[c] = cmul_s<SIGN>(x[c], tab[((c - 1) << LOGM) | b]);
+  }
+}
+
 // One stage on the 16 registers of a thread.
 //   DIF:  x <- Dft(x) then x[c] *= w_L^(SIGN b c)        (L = 2^(LR+LOGM), b = point index mod 2^LOGM)
 //   DIT:  x[c] *= w_L^(SIGN b c) then x <- Dft(x)        (the adjoint of the DIF stage of opposite SIGN)
@@ -181,15 +209,9 @@ __device__ __forceinline__ void stage_math(cpx (&v)[16], int base, const cpx* __
     const int b = ((base | (jq << LO)) >> LOGW) & ((1 << LOGM) - 1);
     if constexpr (DIF) {
       Dft<R, SIGN>::run(x);
-      if constexpr (LOGM > 0) {
-#pragma unroll
-        for (int c = 1; c < R; ++c) x[c] = cmul_s<SIGN>(x[c], tab[((c - 1) << LOGM) | b]);
-      }
+      if constexpr (LOGM > 0) stage_twiddle<R, LR, LOGM, SIGN>(x, tab, b);
     } else {
-      if constexpr (LOGM > 0) {
-#pragma unroll
-        for (int c = 1; c < R; ++c) x[c] = cmul_s<SIGN>(x[c], tab[((c - 1) << LOGM) | b]);
-      }
+      if constexpr (LOGM > 0) stage_twiddle<R, LR, LOGM, SIGN>(x, tab, b);
       Dft<R, SIGN>::run(x);
     }
 #pragma unroll

@@ -238,9 +238,9 @@ k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
 
 // -------------------------------------------------------------------------------------------------------- pass B
 // A "chunk" is one contiguous run of N2 values (memory row p1 of field row r: chunk = r * N1 + p1); a tile is
-// 2^(12 - LOGN2) consecutive chunks.  The exp(h/2 L) table holds, per (mode, p1) chunk, its N2 entries in the
-// register order of the last forward stage: entry [(q & 15) << (LOGN2 - 4) | (q >> 4)] belongs to slot q, so that
-// lanes read consecutive entries.
+// 2^(12 - LOGN2) consecutive chunks = 64 KiB of contiguous memory.  The exp(h/2 L) table holds, per (mode, p1) chunk,
+// its N2 entries in the register order of the last forward stage: entry [(q & 15) << (LOGN2 - 4) | (q >> 4)] belongs
+// to slot q, so that lanes read consecutive entries.
 struct RowsParams {
   cpx* X0;
   cpx* X1;
@@ -250,71 +250,167 @@ struct RowsParams {
   int logn1, nbuf, M;
 };
 
+#define MMF_ROWS_SLOTS 3
+template <int LOGN2>
+__host__ __device__ constexpr size_t rows_smem_bytes() {
+  constexpr int TWN = tw_total_entries(LOGN2, nstages(LOGN2));
+  return sizeof(cpx) * (((size_t)MMF_ROWS_SLOTS << MMF_TILE_LOG) + ((TWN + 7) & ~7)) + 64;
+}
+
 // MODE 0: transform, * E, adjoint transform (in place).  MODE 1: forward transform only, output in slot order
 // (debug entry point).  SINGLE: N1 = 1 (the whole of D in this kernel; tiles may be ragged and hold several rows).
-// Three-pass order of work: an item is (mode a, tile of chunks), its 2 nbuf sub-tiles (polarisation x buffer) share
-// one piece of the table and are done back to back by the same group, so the table is read from HBM once.
+// Order of work: an item is (mode a, tile of chunks); its 2 nbuf sub-tiles (polarisation x buffer) share one piece of
+// the table and are done back to back by the same group, so the table comes from HBM once.  The CTA's items
+// j = 0, 1, ... (item blockIdx.x + j gridDim.x) go to group j % 2.
+// Data movement: as in k_cols — the CTA's tiles tt = 0, 1, ... (group tt % 2, sub-tile (tt / 2) % sub of item
+// 2 (tt / (2 sub)) + tt % 2) rotate through three 64 KiB ring slots that are also the exchange buffers; a tile is one
+// contiguous bulk copy each way (cp.async.bulk), issued by the group's first thread.  The sub-tiles of an odd last
+// item alternate between the groups, so the rotation has no holes.
 template <int LOGN2, int MODE, bool SINGLE, int G>
 __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) {
+  static_assert(G == 2, "two groups alternate over the ring");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   constexpr int LOGB = MMF_TILE_LOG - LOGN2;
   constexpr int NST = nstages(LOGN2);
   constexpr int TWN = tw_total_entries(LOGN2, NST);
   constexpr int LR1 = stage_lr(LOGN2, NST), LO1 = stage_lo(LOGN2 - LR1, 0, MMF_TILE_LOG);
-  cpx* tab = reinterpret_cast<cpx*>(smem_raw);
-  load_stage_tables<TWN>(tab, p.twtab);
+  constexpr int S = MMF_ROWS_SLOTS;
+  constexpr int TILE_BYTES = (int)sizeof(cpx) << MMF_TILE_LOG;
+  cpx* ring = reinterpret_cast<cpx*>(smem_raw);
+  cpx* tab = ring + ((size_t)S << MMF_TILE_LOG);
+  uint64_t* full = reinterpret_cast<uint64_t*>(tab + ((TWN + 7) & ~7));
+  uint64_t* done = full + S;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
+#pragma unroll
+    for (int i = 0; i < G; ++i) mbar_init(&done[i], MMF_GROUP_THREADS);
+    mbar_init_fence();
+  }
+  load_stage_tables<TWN>(tab, p.twtab);  // ends with __syncthreads
   const int grp = threadIdx.x / MMF_GROUP_THREADS, t = threadIdx.x % MMF_GROUP_THREADS;
-  cpx* s = tab + ((TWN + 7) & ~7) + (grp << MMF_TILE_LOG);
+  const bool elect = t == 0;
   const int bar = 1 + grp;
   const int base1 = stage_base<LO1>(t);
   const int cht = (t << 4) >> LOGN2;                 // chunk (inside the tile) of this thread's last-stage values
   const int tq = t & ((1 << (LOGN2 - 4)) - 1);
   const int logn1 = p.logn1;
-  const int sub = SINGLE ? p.nbuf : 2 * p.nbuf;
+  const int logsub = (SINGLE ? 0 : 1) + (p.nbuf > 1 ? 1 : 0);   // sub-tiles per item: nbuf (SINGLE) or 2 nbuf
   const long long items = SINGLE ? ((p.nchunks + (1 << LOGB) - 1) >> LOGB) : ((long long)p.M << (logn1 - LOGB));
-  for (long long item = (long long)blockIdx.x * G + grp; item < items; item += (long long)gridDim.x * G) {
-    for (int sidx = 0; sidx < sub; ++sidx) {
-      long long chunk0, ech;   // first chunk of the tile; table chunk of this thread's last-stage values
-      int buf;
-      if constexpr (SINGLE) {
-        chunk0 = item << LOGB;
-        buf = sidx;
-        ech = (chunk0 + cht) >> 1;  // chunk = row, table chunk = mode
-      } else {
+  const long long nitem = items > blockIdx.x ? (items - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;  // this CTA's
+  const long long npaired = (nitem >> 1) << (logsub + 1);        // tiles of the items done in pairs (one per group)
+  const long long ntile = npaired + ((nitem & 1) << logsub);     // an odd last item: its sub-tiles alternate groups
+
+  // geometry of the CTA's tile tt: first chunk, buffer, item
+  auto tile_geom = [&](long long tt, long long& chunk0, int& buf, long long& item) {
+    long long j;
+    int sidx;
+    if (tt < npaired) {
+      const long long q = tt >> 1;
+      j = ((q >> logsub) << 1) + (tt & 1);
+      sidx = (int)(q & ((1 << logsub) - 1));
+    } else {
+      j = nitem - 1;
+      sidx = (int)(tt - npaired);
+    }
+    item = blockIdx.x + j * gridDim.x;
+    if constexpr (SINGLE) {
+      chunk0 = item << LOGB;
+      buf = sidx;
+    } else {
+      const long long a = item >> (logn1 - LOGB), tau = item & ((1LL << (logn1 - LOGB)) - 1);
+      chunk0 = ((2 * a + (sidx & 1)) << logn1) + (tau << LOGB);
+      buf = sidx >> 1;
+    }
+  };
+  auto tile_bytes = [&](long long chunk0) -> uint32_t {
+    if constexpr (SINGLE) {
+      const long long left = (p.nchunks - chunk0) << LOGN2;
+      return (uint32_t)(left < (1LL << MMF_TILE_LOG) ? left * (long long)sizeof(cpx) : TILE_BYTES);
+    } else {
+      return TILE_BYTES;
+    }
+  };
+  auto issue_load = [&](long long tt) {
+    long long chunk0, item;
+    int buf;
+    tile_geom(tt, chunk0, buf, item);
+    const int b = (int)(tt % S);
+    const uint32_t bytes = tile_bytes(chunk0);
+    mbar_arrive_expect_tx(&full[b], bytes);
+    bulk_load_1d(smem_raw + (size_t)b * TILE_BYTES, (buf ? p.X1 : p.X0) + (chunk0 << LOGN2), bytes, &full[b]);
+    if constexpr (!SINGLE && MODE == 0) {
+      // first sub-tile of an item (polarisation x of buffer 0): pull the item's piece of the table into L2
+      if (buf == 0 && ((chunk0 >> logn1) & 1) == 0) {
         const long long a = item >> (logn1 - LOGB), tau = item & ((1LL << (logn1 - LOGB)) - 1);
-        chunk0 = ((2 * a + (sidx & 1)) << logn1) + (tau << LOGB);
-        buf = sidx >> 1;
-        ech = (a << logn1) + (tau << LOGB) + cht;
+        bulk_prefetch_l2(p.E + (((a << logn1) + (tau << LOGB)) << LOGN2), TILE_BYTES);
       }
-      cpx* g = (buf ? p.X1 : p.X0) + (chunk0 << LOGN2);
-      cpx v[16];
-#pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const int f = base1 | (j << LO1);
-        const bool live = !SINGLE || chunk0 + (f >> LOGN2) < p.nchunks;
-        v[j] = live ? ld_stream(g + f) : make_double2(0.0, 0.0);
-      }
-      fft_dif<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, +1, MODE == 1>(v, s, t, tab, bar);
-      if constexpr (MODE == 0) {
+    }
+  };
+
+  if (threadIdx.x == 0)
+    for (long long tt = 0; tt < S && tt < ntile; ++tt) issue_load(tt);
+
+  // Only the tile number stays live across the transforms: geometry is recomputed where it is needed (the table
+  // pointer after the forward chain, the store address by the first thread) to keep the 16 values in registers.
+  const int ntile_i = (int)ntile;
+  for (int tt = grp; tt < ntile_i; tt += G) {
+    // the slot this group's previous tile (tt - 2) left: refill it with tile tt + 1 once its store has read it
+    const bool refill = elect && tt >= G && tt - G + S < ntile_i;
+    const int b = tt % S;
+    cpx* s = ring + ((size_t)b << MMF_TILE_LOG);
+    mbar_wait(&full[b], (uint32_t)((tt / S) & 1));
+    cpx v[16];
+    tile_lds_linear<LO1>(v, s, base1);
+    if (refill) {
+      tma_store_wait_read();
+      issue_load(tt - G + S);
+    }
+    fft_dif<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, +1, MODE == 1, true>(v, s, t, tab, bar);
+    if constexpr (MODE == 0) {
+      {
+        long long chunk0, item;
+        int buf;
+        tile_geom(tt, chunk0, buf, item);
         if (!SINGLE || chunk0 + cht < p.nchunks) {
+          long long ech;  // table chunk of this thread's last-stage values
+          if constexpr (SINGLE) {
+            ech = (chunk0 + cht) >> 1;  // chunk = row, table chunk = mode
+          } else {
+            const long long a = item >> (logn1 - LOGB), tau = item & ((1LL << (logn1 - LOGB)) - 1);
+            ech = (a << logn1) + (tau << LOGB) + cht;
+          }
           const cpx* e = p.E + (ech << LOGN2) + tq;
 #pragma unroll
           for (int j = 0; j < 16; ++j) v[j] = cmul(v[j], __ldg(e + (j << (LOGN2 - 4))));
         }
-        fft_dit<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, -1, false>(v, s, t, tab, bar);
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const int f = base1 | (j << LO1);
-          if (!SINGLE || chunk0 + (f >> LOGN2) < p.nchunks) st_stream(g + f, v[j]);
-        }
-      } else {
-        if (!SINGLE || chunk0 + cht < p.nchunks) {
-#pragma unroll
-          for (int j = 0; j < 16; ++j) g[(t << 4) + j] = v[j];
-        }
       }
+      fft_dit<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, -1, false>(v, s, t, tab, bar);
+      group_barrier(bar, MMF_GROUP_THREADS);  // everybody has read the last exchange
+      tile_sts_linear<LO1>(v, s, base1);
+      fence_proxy_async_smem();
+      mbar_arrive(&done[grp]);
+      if (elect) {
+        long long chunk0, item;
+        int buf;
+        tile_geom(tt, chunk0, buf, item);
+        mbar_wait(&done[grp], (uint32_t)((tt >> 1) & 1));
+        bulk_store_1d((buf ? p.X1 : p.X0) + (chunk0 << LOGN2), s, tile_bytes(chunk0));
+        tma_store_commit();
+      }
+    } else {
+      long long chunk0, item;
+      int buf;
+      tile_geom(tt, chunk0, buf, item);
+      if (!SINGLE || chunk0 + cht < p.nchunks) {
+        cpx* g = (buf ? p.X1 : p.X0) + (chunk0 << LOGN2);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) g[(t << 4) + j] = v[j];
+      }
+      group_barrier(bar, MMF_GROUP_THREADS);  // the slot may be refilled
     }
   }
+  if (elect) tma_store_wait_all();
 }
 
 // ------------------------------------------------------------------------------------- exp(h/2 L) table, slot order

@@ -84,12 +84,14 @@ int upload_stage_tables(cpx** dptr, int logp) {
   while (nst > 0) {
     const int lr = stage_lr(remain, nst), logm = remain - lr;
     if (logm > 0)
-      for (int c = 1; c < (1 << lr); ++c)
+      for (int c = 1; c < (1 << lr); ++c) {
+        if (tw_compact(lr, logm) && !(c < 4 || (c & 3) == 0)) continue;  // rows c = 1, 2, 3, 4, 8, 12 only
         for (int b = 0; b < (1 << logm); ++b) {
           cpx w;
           root_of_unity((long long)b * c, 1LL << (lr + logm), &w.x, &w.y);
           h.push_back(w);
         }
+      }
     remain = logm;
     --nst;
   }
@@ -237,8 +239,7 @@ int launch_cols(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
 
 template <int LOGN2, int MODE, bool SINGLE>
 int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
-  constexpr int TWN = tw_total_entries(LOGN2, nstages(LOGN2));
-  constexpr size_t smem = sizeof(cpx) * (((TWN + 7) & ~7) + ((size_t)kGroups << MMF_TILE_LOG));
+  constexpr size_t smem = rows_smem_bytes<LOGN2>();
   constexpr int LOGB = MMF_TILE_LOG - LOGN2;
   auto kern = k_rows<LOGN2, MODE, SINGLE, kGroups>;
   static bool attr_done = false;
@@ -251,8 +252,7 @@ int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   q.nchunks = (2LL * p->M) << p->logn1;
   q.logn1 = p->logn1; q.nbuf = nbuf; q.M = p->M;
   const long long items = SINGLE ? ((q.nchunks + (1 << LOGB) - 1) >> LOGB) : ((long long)p->M << (p->logn1 - LOGB));
-  long long grid = (items + kGroups - 1) / kGroups;
-  if (grid > p->num_sms) grid = p->num_sms;
+  long long grid = items < p->num_sms ? items : p->num_sms;
   LaunchTimer lt(p, KC_ROWS, st);
   kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(q);
   p->launches++;
