@@ -167,6 +167,15 @@ __device__ __forceinline__ void tile_sts(const cpx (&v)[16], cpx* __restrict__ s
 __device__ __forceinline__ void group_barrier(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
 }
+// Synchronisation of the exchange between two stage layouts LOA, LOB.  The thread index is the flat index f with the
+// 4 register bits at [LO, LO+4) removed; when both register fields lie below bit 9, f[9:11] is thread bits [5:7] in
+// both layouts, i.e. every value stays inside its warp and __syncwarp is enough — the warps of a group then drift
+// apart between the group-wide exchanges, and one warp's shared-memory phase overlaps another's arithmetic.
+template <int LOA, int LOB>
+__device__ __forceinline__ void exchange_barrier(int id) {
+  if constexpr (LOA <= 5 && LOB <= 5) __syncwarp();
+  else group_barrier(id, MMF_GROUP_THREADS);
+}
 
 // x[c] *= w^(SIGN b c), c = 1 .. R-1, from this stage's table (full: row c-1; compact: see tw_compact)
 template <int R, int LR, int LOGM, int SIGN>
@@ -236,7 +245,7 @@ __device__ __forceinline__ void fft_dif(cpx (&v)[16], cpx* __restrict__ s, int t
     constexpr int LR2 = stage_lr(LOGM, NST - 1), LO2 = stage_lo(LOGM - LR2, LOGW, LOGTOT);
     if constexpr (PRESYNC && REMAIN == LOGP) group_barrier(bar, MMF_GROUP_THREADS);
     tile_sts<LO>(v, s, base);
-    group_barrier(bar, MMF_GROUP_THREADS);
+    exchange_barrier<LO, LO2>(bar);
     tile_lds<LO2>(v, s, stage_base<LO2>(t));
     if constexpr (FENCE && NST == 2) group_barrier(bar, MMF_GROUP_THREADS);
     fft_dif<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, FENCE, PRESYNC>(v, s, t, tab, bar);
@@ -254,7 +263,7 @@ __device__ __forceinline__ void fft_dit(cpx (&v)[16], cpx* __restrict__ s, int t
     fft_dit<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, false, PRESYNC>(v, s, t, tab, bar);
     if constexpr (PRESYNC && NST == 2) group_barrier(bar, MMF_GROUP_THREADS);
     tile_sts<LO2>(v, s, stage_base<LO2>(t));
-    group_barrier(bar, MMF_GROUP_THREADS);
+    exchange_barrier<LO2, LO>(bar);
     tile_lds<LO>(v, s, base);
     if constexpr (FENCE) group_barrier(bar, MMF_GROUP_THREADS);
   }
