@@ -32,6 +32,12 @@ def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the committed `ncu --set full` capture of this
+# command on cfg4 (profiles/r1e_ncu_full_cfg4.md); other workloads have no capture: traffic = null.
+NCU_TRAFFIC_CFG4 = {"k_rows": 75.40e9, "k_cols<fwd>": 65.45e9, "k_cols<inv>": 65.48e9, "k_nlm<s23>": 64.38e9,
+                    "k_nlm<final_next>": 64.37e9}
+
+
 def load_peaks():
     """HBM GB/s of MEASURED_PEAKS.json (driver-written), else the profiling guide's fallback."""
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -265,12 +271,42 @@ def run_mmf(args):
         avg = top["total_ms"] / top["launches"]
         ach = top["alg_bytes_per_launch"] / (avg * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": top["name"], "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                "frac": ach / peak, "traffic": NCU_TRAFFIC_CFG4.get(top["name"]) if args.cfg == 4 else None,
+                "traffic_source": "profiles/r1e_ncu_full_cfg4.md" if args.cfg == 4 else None, "peak_source": peak_src,
                 "alg_bytes_per_launch": top["alg_bytes_per_launch"], "avg_launch_ms": avg}
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
     balg = (36 if p.N > 4096 else 20) * F
     t_roof_ms = balg / (peak * 1e9) * 1e3
     step_roof = {"B_alg_bytes_per_step": balg, "hbm_time_ms": t_roof_ms, "frac": t_roof_ms / (ms / args.steps)}
+
+    # ---- cuFFT (through torch.fft) beside the hand-written transforms: a reference point only, never on the path ----
+    cufft = None
+    if not args.no_cufft and world == 1:
+        try:
+            Ecf = torch.ones((p.M, 1, p.N), dtype=torch.complex128, device=dev)   # stands in for exp(h/2 L)/N
+            Xv = X.view(p.M, 2, p.N)
+
+            def d_cufft():
+                S = torch.fft.fft(Xv, dim=2)
+                S *= Ecf
+                torch.fft.ifft(S, dim=2, out=Xv)
+
+            d_cufft()
+            torch.cuda.synchronize()
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record(stream)
+            for _ in range(3):
+                d_cufft()
+            c1.record(stream)
+            torch.cuda.synchronize()
+            ms_cf = c0.elapsed_time(c1) / 3
+            ours = sum(k["total_ms"] / k["launches"] for k in kern if k["name"] in ("k_cols<fwd>", "k_rows", "k_cols<inv>"))
+            cufft = {"what": "one D = ifft(E * fft(x)) over the whole field with torch.fft (cuFFT, out of place + "
+                             "elementwise multiply)", "ms_per_field": ms_cf,
+                     "ours_ms_per_field": ours / 2 if p.N > 4096 else None}
+            del Ecf
+        except Exception as exc:                     # reference point only: never fail the bench on it
+            cufft = {"unavailable": repr(exc)[:200]}
 
     # ---- the CPU oracle, timed on this box's host cores on a bounded sample ----
     cpu = None
@@ -288,7 +324,7 @@ def run_mmf(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": F / args.steps,
                     "d2h_bytes_per_step": F / args.steps, "ms_per_call": ms_e2e,
                     "call": "mmf_propagate_host(nsteps=%d): one H2D + one D2H of F per call" % args.steps},
-            "gpu_launches": launches, "roofline": roof, "step_roofline": step_roof, "kernels": breakdown,
+            "gpu_launches": launches, "roofline": roof, "step_roofline": step_roof, "kernels": breakdown, "cufft_reference": cufft,
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -304,6 +340,7 @@ def main():
     ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json config id (default 4: M=120, N=2^22)")
     ap.add_argument("--impl", default="mmf", choices=["mmf", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT reference point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     if args.impl == "reference":
