@@ -183,11 +183,9 @@ def run_reference(args):
 def run_mmf(args):
     import numpy as np
     import torch
-    from paper_1901_01895_b200 import binding, workloads
+    from paper_1901_01895_b200 import binding, replicas, workloads
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank, local_rank, world = replicas.env_rank_world()
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -207,6 +205,9 @@ def run_mmf(args):
     log("[bench] input generated in %.1f s" % (time.perf_counter() - t0))
     X = torch.empty((p.R, p.N), dtype=torch.complex128, device=dev)
     X.copy_(H)
+    if world > 1:                                    # replicas: a launch-power sweep, one power per rank
+        X *= replicas.amplitude_scale(rank, world)
+        H.copy_(X)
     plan = binding.Plan(p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, device=dev)
     stream = torch.cuda.current_stream()
 
@@ -233,11 +234,7 @@ def run_mmf(args):
     kern = plan.get_timing()
     plan.set_timing(False)
     clocks = sampler.stop()
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * p.R * p.N * args.steps / (ms * 1e-3)
+    _, ms, value = replicas.whole_job(p.R * p.N * args.steps, ms, dist, dev)
     assert bool(torch.isfinite(X.view(torch.float64)).all()), "propagated field is not finite"
 
     # ---- end to end: host buffer in, host buffer out, through the C ABI ----
@@ -247,11 +244,7 @@ def run_mmf(args):
     e1.record(stream)
     barrier()
     ms_e2e = e0.elapsed_time(e1)                    # device clock over the whole call
-    if dist is not None:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e_value = world * p.R * p.N * args.steps / (ms_e2e * 1e-3)
+    _, ms_e2e, e2e_value = replicas.whole_job(p.R * p.N * args.steps, ms_e2e, dist, dev)
 
     if rank != 0:
         return 0
@@ -319,7 +312,7 @@ def run_mmf(args):
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_string(p), "l2": "field copy %.1f GiB >> 126 MB L2 (no flush needed)"
                        % (F / 2 ** 30) if F > 4 * 126e6 else "working set near/below L2 size: L2-resident",
-                       "parallelism": "replicas x%d (no collective)" % world},
+                       "parallelism": "replicas x%d (launch-power sweep, no collective)" % world},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": F / args.steps,
                     "d2h_bytes_per_step": F / args.steps, "ms_per_call": ms_e2e,
