@@ -93,3 +93,46 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
 }
 
 }  // namespace mmf
+
+// ---- tensor memory (TMEM, 256 KB per SM) used as per-thread scratch ---------------------------------------------
+// With the 32x32b shape every thread of a warp reads / writes consecutive 32-bit columns of ITS OWN lane
+// (lane 32 (warp % 4) + laneid), so TMEM serves as a private, explicitly addressed extension of the register file
+// that costs neither shared-memory space nor LSU bandwidth.  Address = base + (lane << 16) + column.
+namespace mmf {
+
+// one full warp: allocate ncols (power of two >= 32) columns, base address written to *smem_word
+__device__ __forceinline__ void tmem_alloc(uint32_t* smem_word, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(smem_word)),
+               "r"(ncols)
+               : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tmem_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tmem_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n"); }
+
+// two complex doubles (8 columns) of this thread -> its lane at taddr (whole warp, converged).  No "memory" clobber
+// on the data-path wrappers: TMEM is not memory the compiler knows, and global loads must stay free to move.
+__device__ __forceinline__ void tmem_st_c2(uint32_t taddr, const double2 (&e)[2]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};\n" ::"r"(taddr),
+               "r"(__double2loint(e[0].x)), "r"(__double2hiint(e[0].x)), "r"(__double2loint(e[0].y)),
+               "r"(__double2hiint(e[0].y)), "r"(__double2loint(e[1].x)), "r"(__double2hiint(e[1].x)),
+               "r"(__double2loint(e[1].y)), "r"(__double2hiint(e[1].y)));
+}
+// the reverse (waits for the load; the wait names the registers so that no use of them is scheduled ahead of it)
+__device__ __forceinline__ void tmem_ld_c2(double2 (&e)[2], uint32_t taddr) {
+  int r[8];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];\n"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;\n"
+               : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]));
+  e[0] = make_double2(__hiloint2double(r[1], r[0]), __hiloint2double(r[3], r[2]));
+  e[1] = make_double2(__hiloint2double(r[5], r[4]), __hiloint2double(r[7], r[6]));
+}
+
+}  // namespace mmf

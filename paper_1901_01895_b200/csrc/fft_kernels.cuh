@@ -280,6 +280,12 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
   cpx* tab = ring + ((size_t)S << MMF_TILE_LOG);
   uint64_t* full = reinterpret_cast<uint64_t*>(tab + ((TWN + 7) & ~7));
   uint64_t* done = full + S;
+  // The E values of a thread are the same for the 2 nbuf sub-tiles of an item: the first sub-tile takes them from
+  // global memory and parks them in tensor memory (64 columns of the thread's own lane), the others read them back
+  // from there — no global-load latency, no LSU traffic, no shared memory (none is left).
+  constexpr bool ECACHE = MODE == 0 && !SINGLE;
+  constexpr uint32_t TMEM_COLS = 256;  // 4 warps share a lane quarter: 4 x 64 columns
+  uint32_t* tmem_word = reinterpret_cast<uint32_t*>(done + G);
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
@@ -287,7 +293,18 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
     for (int i = 0; i < G; ++i) mbar_init(&done[i], MMF_GROUP_THREADS);
     mbar_init_fence();
   }
+  if constexpr (ECACHE) {
+    if (threadIdx.x < 32) tmem_alloc(tmem_word, TMEM_COLS);
+    tmem_fence_before_sync();
+  }
   load_stage_tables<TWN>(tab, p.twtab);  // ends with __syncthreads
+  uint32_t taddr = 0;
+  if constexpr (ECACHE) {
+    tmem_fence_after_sync();
+    const uint32_t warp = threadIdx.x >> 5;
+    taddr = *tmem_word + (((warp & 3) * 32) << 16) + (warp >> 2) * 64;
+  }
+  int cached_item = -1;
   const int grp = threadIdx.x / MMF_GROUP_THREADS, t = threadIdx.x % MMF_GROUP_THREADS;
   const bool elect = t == 0;
   const int bar = 1 + grp;
@@ -381,8 +398,32 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
             ech = (a << logn1) + (tau << LOGB) + cht;
           }
           const cpx* e = p.E + (ech << LOGN2) + tq;
+          if constexpr (ECACHE) {
+            if ((int)item == cached_item) {  // uniform over the group
 #pragma unroll
-          for (int j = 0; j < 16; ++j) v[j] = cmul(v[j], __ldg(e + (j << (LOGN2 - 4))));
+              for (int c = 0; c < 8; ++c) {
+                cpx ev[2];
+                tmem_ld_c2(ev, taddr + 8 * c);
+                v[2 * c] = cmul(v[2 * c], ev[0]);
+                v[2 * c + 1] = cmul(v[2 * c + 1], ev[1]);
+              }
+            } else {
+#pragma unroll
+              for (int c = 0; c < 8; ++c) {
+                cpx ev[2];
+                ev[0] = __ldg(e + ((2 * c) << (LOGN2 - 4)));
+                ev[1] = __ldg(e + ((2 * c + 1) << (LOGN2 - 4)));
+                tmem_st_c2(taddr + 8 * c, ev);
+                v[2 * c] = cmul(v[2 * c], ev[0]);
+                v[2 * c + 1] = cmul(v[2 * c + 1], ev[1]);
+              }
+              tmem_wait_st();
+              cached_item = (int)item;
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = cmul(v[j], __ldg(e + (j << (LOGN2 - 4))));
+          }
         }
       }
       fft_dit<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, -1, false>(v, s, t, tab, bar);
@@ -411,6 +452,11 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
     }
   }
   if (elect) tma_store_wait_all();
+  if constexpr (ECACHE) {
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (threadIdx.x < 32) tmem_dealloc(*tmem_word, TMEM_COLS);
+  }
 }
 
 // ------------------------------------------------------------------------------------- exp(h/2 L) table, slot order
