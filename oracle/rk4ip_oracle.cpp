@@ -229,6 +229,25 @@ void rk4ip_step(cplx* A, int M, long long N, const cplx* E, double hgamma, const
   for (long long i = 0; i < tot; ++i) A[i] = tmp[i] + k4[i] / 6.0;
 }
 
+// One symmetric split step with a Runge-Kutta nonlinear substep ("SSFM-RK4": Eq. 4 PAPER.md:58-61 with the nonlinear
+// part "solved ... with explicit schemes like the Runge-Kutta method"), written out in that order:
+//   A <- exp(h/2 L) A;   A <- classical RK4 over h of dA/dz = N(A) A (Eq. 1 without its linear part);   A <- exp(h/2 L) A
+// E is the table for hh = h/2; hgamma = h*gamma, so nonlinear() returns h N(u) u.  Plain buffers, nothing fused.
+void ssfm_rk4_step(cplx* A, int M, long long N, const cplx* E, double hgamma, const double* kappa, int nthreads,
+                   cplx* k1, cplx* k2, cplx* k3, cplx* k4, cplx* tmp) {
+  const long long tot = 2LL * M * N;
+  apply_D(A, M, N, E, nthreads);
+  nonlinear(A, k1, M, N, hgamma, kappa, nthreads);
+  for (long long i = 0; i < tot; ++i) tmp[i] = A[i] + k1[i] / 2.0;
+  nonlinear(tmp, k2, M, N, hgamma, kappa, nthreads);
+  for (long long i = 0; i < tot; ++i) tmp[i] = A[i] + k2[i] / 2.0;
+  nonlinear(tmp, k3, M, N, hgamma, kappa, nthreads);
+  for (long long i = 0; i < tot; ++i) tmp[i] = A[i] + k3[i];
+  nonlinear(tmp, k4, M, N, hgamma, kappa, nthreads);
+  for (long long i = 0; i < tot; ++i) A[i] = A[i] + k1[i] / 6.0 + k2[i] / 3.0 + k3[i] / 3.0 + k4[i] / 6.0;
+  apply_D(A, M, N, E, nthreads);
+}
+
 }  // namespace
 
 extern "C" {
@@ -287,6 +306,20 @@ int orc_rk4ip(double* A, int M, long long N, double dt, double h, double alpha, 
   for (int s = 0; s < nsteps; ++s)
     rk4ip_step((cplx*)A, M, N, E.data(), h * gamma, kappa, nthreads, AI.data(), k1.data(), k2.data(), k3.data(),
                k4.data(), tmp.data());
+  return 0;
+}
+
+// A[2M][N] advanced nsteps SSFM-RK4 steps of size h (symmetric split step, Eq. 4), in place.
+int orc_ssfm_rk4(double* A, int M, long long N, double dt, double h, double alpha, const double* beta, int K,
+                 double gamma, const double* kappa, int nsteps, int nthreads) {
+  if (!A || !beta || !kappa || M < 1 || K < 1 || !is_pow2(N) || !(dt > 0) || nsteps < 0) return -1;
+  if (nsteps == 0) return 0;
+  const long long tot = 2LL * M * N;
+  std::vector<cplx> E((size_t)M * N), k1(tot), k2(tot), k3(tot), k4(tot), tmp(tot);
+  linear_table(E.data(), M, N, dt, h / 2.0, alpha, beta, K, nthreads);
+  for (int s = 0; s < nsteps; ++s)
+    ssfm_rk4_step((cplx*)A, M, N, E.data(), h * gamma, kappa, nthreads, k1.data(), k2.data(), k3.data(), k4.data(),
+                  tmp.data());
   return 0;
 }
 

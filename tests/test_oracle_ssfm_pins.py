@@ -1,0 +1,109 @@
+"""Pins of the oracle's SSFM-RK4 step (symmetric split step, Eq. 4) against what the
+equation and the mathematics fix — not against the oracle itself:
+  * gamma = 0: the split is exact, the step is exp(h L) (closed-form spectral solution of Eq. 1, written in numpy);
+  * alpha = beta = 0: the linear half steps are the identity and the nonlinear substep is classical RK4 on a
+    per-sample ODE whose exact solution is a phase rotation: error x16 per halving;
+  * the whole of Eq. (1) against an independent adaptive integration (scipy DOP853, spectral right-hand side written
+    separately): "a global error of O(h^2)": error x4 per halving — and RK4IP at the same step size is
+    more accurate (the paper's reason for RK4IP);
+  * composition n1 + n2 steps is bit-identical to n1 + n2 at once; a zero field stays zero.
+"""
+import math
+
+import numpy as np
+
+
+def rel(x, ref):
+    return float(np.linalg.norm(np.ravel(x - ref)) / max(np.linalg.norm(np.ravel(ref)), 1e-300))
+
+
+def rand_c(rng, *shape):
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+def eq1_linear_symbol(w_np, alpha, beta_a):
+    """L of Eq. (1) as printed (time domain), acting on exp(+i w t): d/dt -> (i w)."""
+    L = np.full(w_np.shape, -alpha / 2.0, dtype=complex)
+    for n, b in enumerate(beta_a):
+        L = L + 1j * (1j ** n) / math.factorial(n) * b * (1j * w_np) ** n
+    return L
+
+
+def test_gamma_zero_is_the_exact_linear_solution(orc):
+    M, N, dt, h, steps = 2, 64, 0.7, 3.0, 5
+    rng = np.random.default_rng(3)
+    X = rand_c(rng, 2 * M, N)
+    X[:, N // 2] = 0            # the Nyquist bin's frequency sign is a convention (reading R7)
+    A = np.fft.ifft(X, axis=1)
+    alpha = 0.02
+    beta = np.array([[0.01, 0.03, -0.05, 0.004], [-0.02, -0.01, -0.03, 0.002]])
+    w = 2 * np.pi * np.fft.fftfreq(N, d=dt)
+    want = np.empty_like(A)
+    for r in range(2 * M):
+        want[r] = np.fft.ifft(np.exp(eq1_linear_symbol(w, alpha, beta[r // 2]) * h * steps) * np.fft.fft(A[r]))
+    got = orc.ssfm_rk4(A, dt, h, alpha, beta, 0.0, np.eye(M), steps, nthreads=1)
+    assert rel(got, want) <= 1e-13
+
+
+def test_no_dispersion_is_rk4_on_the_phase_rotation(orc):
+    M, N, dt = 3, 32, 1.0
+    rng = np.random.default_rng(19)
+    A = rand_c(rng, 2 * M, N) * np.array([1.0, 0.3, 0.7, 1.4, 0.2, 0.9])[:, None]
+    kappa = rng.uniform(0.1, 1.0, size=(M, M))          # non-symmetric: catches a transposed kappa
+    gamma, z = 0.9, 0.15
+    S = kappa @ (np.abs(A[0::2]) ** 2 + np.abs(A[1::2]) ** 2)
+    want = A * np.exp(1j * gamma * np.repeat(S, 2, axis=0) * z)
+    errs = [rel(orc.ssfm_rk4(A, dt, z / n, 0.0, np.zeros((M, 1)), gamma, kappa, n, nthreads=1), want)
+            for n in (4, 8, 16, 32)]
+    ratios = [errs[i] / errs[i + 1] for i in range(3)]
+    assert errs[-1] < 1e-5
+    assert all(12.0 < r < 20.0 for r in ratios[1:]), ratios
+
+
+def test_second_order_global_error_against_independent_solution_of_eq1(orc):
+    from scipy.integrate import solve_ivp
+    M, N, dt, z = 2, 128, 1.0, 120.0
+    rng = np.random.default_rng(77)
+    X = np.zeros((2 * M, N), dtype=complex)
+    X[:, :4] = rand_c(rng, 2 * M, 4)
+    X[:, -3:] = rand_c(rng, 2 * M, 3)
+    A0 = np.fft.ifft(X, axis=1) * (N / 32) * np.array([9.0, 3.6, 6.6, 10.5])[:, None]
+    alpha, gamma = 2e-3, 1.7e-3
+    beta = np.array([[4e-3, 9e-3, -25e-3, 3e-3], [-6e-3, -7e-3, -18e-3, -2e-3]])
+    kappa = np.array([[1.0, 0.35], [0.8, 0.6]])
+    w = 2 * np.pi * np.fft.fftfreq(N, d=dt)
+    Lsym = np.vstack([eq1_linear_symbol(w, alpha, beta[r // 2]) for r in range(2 * M)])
+
+    def rhs(_z, y):
+        A = (y[: y.size // 2] + 1j * y[y.size // 2:]).reshape(2 * M, N)
+        lin = np.fft.ifft(Lsym * np.fft.fft(A, axis=1), axis=1)
+        P = np.abs(A[0::2]) ** 2 + np.abs(A[1::2]) ** 2
+        d = (lin + 1j * gamma * np.repeat(kappa @ P, 2, axis=0) * A).ravel()
+        return np.concatenate([d.real, d.imag])
+
+    y0 = np.concatenate([A0.ravel().real, A0.ravel().imag])
+    sol = solve_ivp(rhs, (0.0, z), y0, method="DOP853", rtol=1e-12, atol=1e-14)
+    assert sol.success
+    ref = (sol.y[: y0.size // 2, -1] + 1j * sol.y[y0.size // 2:, -1]).reshape(2 * M, N)
+    errs = [rel(orc.ssfm_rk4(A0, dt, z / n, alpha, beta, gamma, kappa, n, nthreads=1), ref) for n in (32, 64, 128, 256)]
+    ratios = [errs[i] / errs[i + 1] for i in range(3)]
+    assert errs[-1] < 1e-3, errs
+    assert all(3.5 < r < 4.5 for r in ratios), (errs, ratios)           # O(h^2) globally
+    # the interaction-picture scheme has no splitting error: at the same step size it is far more accurate
+    err_ip = rel(orc.rk4ip(A0, dt, z / 128, alpha, beta, gamma, kappa, 128, nthreads=1), ref)
+    assert err_ip < 1e-2 * errs[2]
+
+
+def test_composition_and_zero_field(orc):
+    M, N, dt, h = 2, 32, 1.0, 2.0
+    rng = np.random.default_rng(5)
+    A = rand_c(rng, 2 * M, N) * 0.3
+    A[1] = 0
+    beta = np.array([[0.0, 0.01, -0.02, 0.001], [0.0, -0.01, -0.03, 0.001]])
+    kappa = np.array([[1.0, 0.4], [0.4, 1.0]])
+    a = orc.ssfm_rk4(orc.ssfm_rk4(A, dt, h, 1e-3, beta, 0.5, kappa, 2, nthreads=1), dt, h, 1e-3, beta, 0.5, kappa, 3,
+                     nthreads=1)
+    b = orc.ssfm_rk4(A, dt, h, 1e-3, beta, 0.5, kappa, 5, nthreads=1)
+    assert np.array_equal(a, b)
+    assert np.all(b[1] == 0) and np.any(b[0] != 0)
+    assert np.array_equal(orc.ssfm_rk4(A, dt, h, 1e-3, beta, 0.5, kappa, 0), A)
