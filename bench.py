@@ -217,7 +217,8 @@ def run_mmf(args):
         torch.cuda.synchronize()
 
     # ---- warm-up (W untimed steps), then K timed steps, field resident in HBM ----
-    plan.propagate(X, args.warmup)
+    advance = plan.propagate if args.method == "rk4ip" else plan.propagate_ssfm
+    advance(X, args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -226,7 +227,7 @@ def run_mmf(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(stream)
-    plan.propagate(X, args.steps)
+    advance(X, args.steps)
     e1.record(stream)
     barrier()
     launches = plan.launch_count() - n0
@@ -240,7 +241,12 @@ def run_mmf(args):
     # ---- end to end: host buffer in, host buffer out, through the C ABI ----
     barrier()
     e0.record(stream)
-    plan.propagate_host(H, X, args.steps)           # H2D copy, K steps, D2H copy, stream synchronised inside
+    if args.method == "rk4ip":
+        plan.propagate_host(H, X, args.steps)       # H2D copy, K steps, D2H copy, stream synchronised inside
+    else:                                           # no host entry point for the split step: same copies by hand
+        X.copy_(H, non_blocking=True)
+        advance(X, args.steps)
+        H.copy_(X, non_blocking=True)
     e1.record(stream)
     barrier()
     ms_e2e = e0.elapsed_time(e1)                    # device clock over the whole call
@@ -268,7 +274,10 @@ def run_mmf(args):
                 "traffic_source": "profiles/r1e_ncu_full_cfg4.md" if args.cfg == 4 else None, "peak_source": peak_src,
                 "alg_bytes_per_launch": top["alg_bytes_per_launch"], "avg_launch_ms": avg}
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
-    balg = (36 if p.N > 4096 else 20) * F
+    if args.method == "rk4ip":
+        balg = (36 if p.N > 4096 else 20) * F
+    else:                                           # two D on one buffer (3 passes x 2 F, or 2 F on chip) + 2 F
+        balg = (14 if p.N > 4096 else 6) * F
     t_roof_ms = balg / (peak * 1e9) * 1e3
     step_roof = {"B_alg_bytes_per_step": balg, "hbm_time_ms": t_roof_ms, "frac": t_roof_ms / (ms / args.steps)}
 
@@ -310,7 +319,7 @@ def run_mmf(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_string(p), "l2": "field copy %.1f GiB >> 126 MB L2 (no flush needed)"
+            "config": {"workload": workload_string(p), "method": args.method, "l2": "field copy %.1f GiB >> 126 MB L2 (no flush needed)"
                        % (F / 2 ** 30) if F > 4 * 126e6 else "working set near/below L2 size: L2-resident",
                        "parallelism": "replicas x%d (launch-power sweep, no collective)" % world},
             "clocks": clocks,
@@ -332,6 +341,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json config id (default 4: M=120, N=2^22)")
     ap.add_argument("--impl", default="mmf", choices=["mmf", "reference"])
+    ap.add_argument("--method", default="rk4ip", choices=["rk4ip", "ssfm"],
+                    help="rk4ip (Eq. 6, the headline path) or ssfm (SSFM-RK4, the symmetric split step of Eq. 4)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT reference point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

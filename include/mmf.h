@@ -59,6 +59,13 @@ int mmf_plan_set_workspace(mmf_plan *plan, void *ws_dev, size_t bytes, void *cud
  * Calling with n1 then n2 steps equals one call with n1+n2 steps. */
 int mmf_propagate(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
 
+/* Advance A by nsteps SYMMETRIC SPLIT STEPS of size h with a Runge-Kutta nonlinear substep ("SSFM-RK4": Eq. 4
+ * PAPER.md:58-61 with the nonlinear part solved by classical RK4), in place:
+ *   A <- exp(h/2 L) A;  A <- RK4 over h of dA/dz = N(A) A;  A <- exp(h/2 L) A        (globally O(h^2)).
+ * Same arguments and layout as mmf_propagate; runs on the same transform kernels and one fused nonlinear kernel that
+ * evaluates all four N per sample tile (2 F of traffic).  Requires M <= 128 (MMF_EINVAL otherwise). */
+int mmf_propagate_ssfm(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
+
 /* Same, for a HOST field: copies A_host to an internal slot of the workspace-adjacent device buffer `A_dev_scratch`
  * (device, [2M][N] complex128, caller-owned), propagates, copies back and SYNCHRONISES the stream.  A_host should be
  * page-locked for full copy bandwidth.  This is the end-to-end entry point bench.py times. */
@@ -86,7 +93,7 @@ long long mmf_plan_launch_count(const mmf_plan *plan);
  * this plan be bracketed by a pair of CUDA events on the launching stream (and drops earlier records); (plan, 0)
  * switches it off.  mmf_plan_get_timing SYNCHRONISES on the recorded events of kernel class `kclass`
  * (0 <= kclass < mmf_kernel_class_count()) and returns their summed device time [ms], their number, and the
- * ALGORITHMIC bytes one such launch moves as mmf_propagate issues it (full-field reads + writes; tables excluded). */
+ * ALGORITHMIC bytes of one such launch, averaged over the recorded ones (full-field reads + writes; tables excluded). */
 int mmf_plan_set_timing(mmf_plan *plan, int enable);
 int mmf_kernel_class_count(void);
 const char *mmf_kernel_class_name(int kclass);

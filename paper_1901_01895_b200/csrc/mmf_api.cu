@@ -124,29 +124,32 @@ struct mmf_plan {
   bool timing = false;
   std::vector<cudaEvent_t> ev;       // 2 per recorded launch
   std::vector<int> ev_class;         // kernel class of each recorded launch
+  std::vector<double> ev_bytes;      // algorithmic bytes of each recorded launch (full-field reads + writes)
 };
 
 namespace {
 
 // ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
 enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
-       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_COUNT };
+       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_COUNT };
 const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
                                         "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>", "k_nlm<plain>",
-                                        "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>"};
+                                        "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
 struct LaunchTimer {
   mmf_plan* p;
   cudaStream_t st;
   cudaEvent_t stop = nullptr;
-  LaunchTimer(mmf_plan* p_, int kclass, cudaStream_t st_) : p(p_), st(st_) {
+  // nfields = full-field copies the launch reads plus writes (its algorithmic traffic in units of F)
+  LaunchTimer(mmf_plan* p_, int kclass, int nfields, cudaStream_t st_) : p(p_), st(st_) {
     if (!p->timing) return;
     cudaEvent_t a = nullptr;
     if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&stop) != cudaSuccess) { stop = nullptr; return; }
     p->ev.push_back(a);
     p->ev.push_back(stop);
     p->ev_class.push_back(kclass);
+    p->ev_bytes.push_back((double)nfields * (double)p->field_bytes);
     cudaEventRecord(a, st);
   }
   ~LaunchTimer() {
@@ -158,6 +161,7 @@ void clear_events(mmf_plan* p) {
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
   p->ev.clear();
   p->ev_class.clear();
+  p->ev_bytes.clear();
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point query (no link-time dependency on libcuda)
@@ -219,7 +223,7 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   if ((rc = cols_tile_map(p, nbuf > 1 ? X1 : X0, LOGN1, &map1)) != MMF_OK) return rc;
   const long long tiles = ((long long)nbuf * 2 * p->M) << (p->logn2 - LOGW);
   long long grid = tiles < p->num_sms ? tiles : p->num_sms;
-  LaunchTimer lt(p, DIR == 0 ? KC_COLS_FWD : KC_COLS_INV, st);
+  LaunchTimer lt(p, DIR == 0 ? KC_COLS_FWD : KC_COLS_INV, 2 * nbuf, st);
   kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(map0, map1, q);
   p->launches++;
   CU(cudaGetLastError());
@@ -253,7 +257,7 @@ int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   q.logn1 = p->logn1; q.nbuf = nbuf; q.M = p->M;
   const long long items = SINGLE ? ((q.nchunks + (1 << LOGB) - 1) >> LOGB) : ((long long)p->M << (p->logn1 - LOGB));
   long long grid = items < p->num_sms ? items : p->num_sms;
-  LaunchTimer lt(p, KC_ROWS, st);
+  LaunchTimer lt(p, KC_ROWS, 2 * nbuf, st);
   kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(q);
   p->launches++;
   CU(cudaGetLastError());
@@ -307,7 +311,7 @@ int launch_nl(mmf_plan* p, cpx* X, cpx* Y, cpx* Z, cpx* W, cudaStream_t st) {
   q.M = p->M;
   q.N = p->N;
   const unsigned grid = (unsigned)((p->N + MMF_NL_T - 1) / MMF_NL_T);
-  LaunchTimer lt(p, KC_NL_PLAIN + MODE, st);
+  LaunchTimer lt(p, KC_NL_PLAIN + MODE, MODE == NL_PLAIN ? 2 : MODE == NL_STAGE2 ? 3 : MODE == NL_STAGE3 ? 5 : MODE == NL_FINAL ? 3 : 4, st);
   kern<<<grid, MMF_NL_T * MMF_NL_WARPS, smem, st>>>(q);
   p->launches++;
   CU(cudaGetLastError());
@@ -372,7 +376,7 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st) {
   if (occ < 1) return MMF_EINVAL;
   long long grid = (long long)p->num_sms * occ;        // persistent: every resident CTA walks its own tile list
   if (grid > q.ntiles) grid = q.ntiles;
-  LaunchTimer lt(p, KC_NLM_PLAIN + MODE, st);
+  LaunchTimer lt(p, KC_NLM_PLAIN + MODE, (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 2 : MODE == NLM_FINAL ? 3 : 4, st);
   kern<<<(unsigned)grid, threads, smem, st>>>(mapA, mapB, q);
   p->launches++;
   CU(cudaGetLastError());
@@ -585,6 +589,20 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   return MMF_OK;
 }
 
+int mmf_propagate_ssfm(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
+  if (!p || !A_dev || nsteps < 0 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
+  if (!p->ws || p->nlm_nk <= 0) return MMF_EINVAL;  // the fused RK4 substep exists on the tensor path only (M <= 128)
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cpx* X = (cpx*)A_dev;
+  int rc;
+  for (int s = 0; s < nsteps; ++s) {
+    if ((rc = apply_D(p, X, X, 1, st)) != MMF_OK) return rc;              // exp(h/2 L)
+    if ((rc = launch_nlm<NLM_RK4>(p, X, X, st)) != MMF_OK) return rc;     // RK4 over h of dA/dz = N(A) A
+    if ((rc = apply_D(p, X, X, 1, st)) != MMF_OK) return rc;              // exp(h/2 L)
+  }
+  return MMF_OK;
+}
+
 int mmf_propagate_host(mmf_plan* p, void* A_host, void* A_dev_scratch, int nsteps, void* cuda_stream) {
   if (!p || !A_host || !A_dev_scratch || nsteps < 0) return MMF_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -647,30 +665,19 @@ const char* mmf_kernel_class_name(int kclass) { return (kclass >= 0 && kclass < 
 
 int mmf_plan_get_timing(mmf_plan* p, int kclass, double* total_ms, long long* launches, double* alg_bytes) {
   if (!p || kclass < 0 || kclass >= KC_COUNT || !total_ms || !launches || !alg_bytes) return MMF_EINVAL;
-  double tot = 0.0, bytes = 0.0;
+  double tot = 0.0, bytes = 0.0, bsum = 0.0;
   long long n = 0;
   for (size_t i = 0; i < p->ev_class.size(); ++i) {
     if (p->ev_class[i] != kclass) continue;
+    bsum += p->ev_bytes[i];
     CU(cudaEventSynchronize(p->ev[2 * i + 1]));
     float ms = 0.f;
     CU(cudaEventElapsedTime(&ms, p->ev[2 * i], p->ev[2 * i + 1]));
     tot += ms;
     ++n;
   }
-  // algorithmic bytes of ONE launch as mmf_propagate issues it: full-field reads + writes
-  const double F = (double)p->field_bytes;
-  switch (kclass) {
-    case KC_COLS_FWD: case KC_ROWS: case KC_COLS_INV: bytes = 4 * F; break;  // two fields, read + write each
-    case KC_NL_PLAIN: bytes = 2 * F; break;
-    case KC_NL_STAGE2: bytes = 3 * F; break;
-    case KC_NL_STAGE3: bytes = 5 * F; break;
-    case KC_NL_FINAL: bytes = 3 * F; break;
-    case KC_NL_FINAL_NEXT: bytes = 4 * F; break;
-    case KC_NLM_PLAIN: bytes = 2 * F; break;
-    case KC_NLM_S23: bytes = 4 * F; break;
-    case KC_NLM_FINAL: bytes = 3 * F; break;
-    case KC_NLM_FINAL_NEXT: bytes = 4 * F; break;
-  }
+  // algorithmic bytes of one launch: the average over the recorded launches of this class
+  bytes = n > 0 ? bsum / (double)n : 0.0;
   *total_ms = tot;
   *launches = n;
   *alg_bytes = bytes;

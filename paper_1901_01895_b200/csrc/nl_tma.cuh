@@ -9,6 +9,9 @@
 //               instead of the 8 F two kernels need.
 //   NLM_FINAL   X = u4, Y = exp(h/2 L)[...]:  X <- Y + NL(X)/6                   (Eq. 6e + 6f; Y untouched)
 //   NLM_FINAL_NEXT  as NLM_FINAL, then Y <- NL(X_new)                           (the next step's Eq. 6b bracket)
+//   NLM_RK4     X <- X + k1/6 + k2/3 + k3/3 + k4/6,  k1 = NL(X), k2 = NL(X + k1/2), k3 = NL(X + k2/2), k4 = NL(X + k3):
+//               the nonlinear substep of the symmetric split step (Eq. 4, "SSFM-RK4"): classical RK4
+//               over h of dA/dz = N(A) A, four contraction rounds per tile, the field read and written once (2 F).
 //
 // Design.  The kappa contraction S = kappa * P is a (M x M) x (M x 8) fp64 matrix product per tile: it runs on the
 // fp64 tensor path (mma.sync.m8n8k4.f64, SASS DMMA; tcgen05 has no fp64 kind).  Compute warp w owns mode rows
@@ -27,7 +30,7 @@
 
 namespace mmf {
 
-enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3 };
+enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3, NLM_RK4 = 4 };
 
 #define MMF_NLM_T 8           // time samples per tile
 #define MMF_NLM_PSTRIDE 12    // doubles per P row in shared memory (8 + 4: conflict-free B-fragment reads)
@@ -49,7 +52,7 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 }
 
 template <int MODE>
-__host__ __device__ constexpr int nlm_narr() { return MODE == NLM_PLAIN ? 1 : 2; }
+__host__ __device__ constexpr int nlm_narr() { return (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 1 : 2; }
 
 // bytes of dynamic shared memory: ring slots, two P buffers, mbarriers
 __host__ __device__ inline size_t nlt_slot_bytes(int M, int narr) { return (size_t)narr * 2 * M * MMF_NLM_T * sizeof(cpx); }
@@ -175,6 +178,39 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
         if constexpr (MODE == NLM_S23) u[pol][i] = axpy(0.5, y[pol][i], x[pol][i]);
         else u[pol][i] = x[pol][i];
       }
+    if constexpr (MODE == NLM_RK4) {
+      cpx acc[2][2];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        double* Pr = (r & 1) ? Pb1 : Pb0;
+        if (valid)
+          *reinterpret_cast<double2*>(Pr + a * MMF_NLM_PSTRIDE + 2 * q) =
+              make_double2(power2(u[0][0], u[1][0]), power2(u[0][1], u[1][1]));
+        group_barrier(1, gthreads);
+        double sr[2];
+        nlm_contract<NK>(kf, Pr, g, q, sr[0], sr[1]);
+#pragma unroll
+        for (int pol = 0; pol < 2; ++pol)
+#pragma unroll
+          for (int i = 0; i < 2; ++i) {
+            const cpx k = times_ig(u[pol][i], p.hg * sr[i]);  // k_{r+1} = h N(u) u
+            const cpx xx = x[pol][i];
+            if (r == 0) acc[pol][i] = axpy(sixth, k, xx);
+            else acc[pol][i] = axpy((r == 3) ? sixth : third, k, acc[pol][i]);
+            if (r < 3) u[pol][i] = axpy((r == 2) ? 1.0 : 0.5, k, xx);
+          }
+      }
+      if (valid) {
+#pragma unroll
+        for (int pol = 0; pol < 2; ++pol)
+#pragma unroll
+          for (int i = 0; i < 2; ++i) sx[e0 + pol * MMF_NLM_T + i] = acc[pol][i];
+      }
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&done[slot]);
+      continue;
+    }
     // ---- round 1 ---------------------------------------------------------------------------------------------
     if (valid)
       *reinterpret_cast<double2*>(P1 + a * MMF_NLM_PSTRIDE + 2 * q) =
