@@ -63,7 +63,7 @@ int mmf_propagate(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
  * PAPER.md:58-61 with the nonlinear part solved by classical RK4), in place:
  *   A <- exp(h/2 L) A;  A <- RK4 over h of dA/dz = N(A) A;  A <- exp(h/2 L) A        (globally O(h^2)).
  * Same arguments and layout as mmf_propagate; runs on the same transform kernels and one fused nonlinear kernel that
- * evaluates all four N per sample tile (2 F of traffic).  Requires M <= 128 (MMF_EINVAL otherwise). */
+ * evaluates all four N per sample tile (2 F of traffic).  Requires M <= 120 (MMF_EINVAL otherwise). */
 int mmf_propagate_ssfm(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
 
 /* Same, for a HOST field: copies A_host to an internal slot of the workspace-adjacent device buffer `A_dev_scratch`

@@ -591,7 +591,7 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
 
 int mmf_propagate_ssfm(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   if (!p || !A_dev || nsteps < 0 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
-  if (!p->ws || p->nlm_nk <= 0) return MMF_EINVAL;  // the fused RK4 substep exists on the tensor path only (M <= 128)
+  if (!p->ws || p->nlm_nk <= 0) return MMF_EINVAL;  // the fused RK4 substep exists on the tensor path only (M <= 120)
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cpx* X = (cpx*)A_dev;
   int rc;

@@ -1,5 +1,5 @@
 // nl_simt.cuh — the fused nonlinear kernel on the plain FP64 pipe (DFMA), used when M exceeds what the tensor-path
-// kernel of nl_mma.cuh keeps in registers (M > 128).  Rows a4-a7 of the hot-path table.
+// kernel of nl_tma.cuh keeps in registers (M > 120).  Rows a4-a7 of the hot-path table.
 #pragma once
 #include "fft_core.cuh"
 

@@ -34,7 +34,7 @@ enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3, NLM_RK4 = 
 
 #define MMF_NLM_T 8           // time samples per tile
 #define MMF_NLM_PSTRIDE 12    // doubles per P row in shared memory (8 + 4: conflict-free B-fragment reads)
-#define MMF_NLM_MAXM 128      // kappa slab per warp: M/4 doubles per lane -> 16 warps x 8 rows; TMA box <= 256 rows
+#define MMF_NLM_MAXM 120      // 15 compute warps x 8 modes + the producer warp = 512 threads; TMA box <= 256 rows
 #define MMF_NLM_SLOTS 3       // ring depth
 
 struct NltParams {

@@ -114,7 +114,7 @@ def test_linear_operator_white_input_all_bins(mmf, torch, orc):
 
 
 # --------------------------------------------------------------------------------------------- nonlinear operator
-@pytest.mark.parametrize("M,N", [(1, 16), (5, 64), (37, 128), (120, 96 * 0 + 256)])
+@pytest.mark.parametrize("M,N", [(1, 16), (5, 64), (8, 64), (24, 32), (37, 128), (120, 256), (121, 16), (130, 32)])
 def test_nonlinear_operator_integer_exact(mmf, torch, orc, M, N):
     """P10 ii: Gaussian-integer field, integer NON-symmetric kappa, h*gamma = 1: bit-exact against the oracle."""
     rng = np.random.default_rng(M * 1000 + N)
@@ -153,6 +153,7 @@ CASES = [
     (3, 120, 13, 4),
     (4, 120, 14, 3),
     (4, 7, 18, 3),        # config-4 physics at the 2^18 transform size, odd mode count
+    (3, 124, 13, 2),      # more than 120 modes: the DFMA nonlinear kernels and the four-buffer plan
 ]
 
 
