@@ -195,7 +195,7 @@ def run_mmf(args):
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
 
-    p = workloads.problem(args.cfg)
+    p = workloads.problem(args.cfg, M=args.modes, N=None if args.logn is None else 1 << args.logn)
     F = p.R * p.N * 16
     log("[bench] rank %d/%d: %s, field copy F = %.2f GiB" % (rank, world, workload_string(p), F / 2 ** 30))
     t0 = time.perf_counter()
@@ -257,6 +257,7 @@ def run_mmf(args):
 
     # ---- roofline of the dominant kernel (largest summed device time in the timed region) ----
     peak, peak_src = load_peaks()
+    full_cfg4 = args.cfg == 4 and args.modes is None and args.logn is None and args.method == "rk4ip"
     roof = None
     breakdown = []
     tot_kernel_ms = sum(k["total_ms"] for k in kern) or 1.0
@@ -270,8 +271,8 @@ def run_mmf(args):
         avg = top["total_ms"] / top["launches"]
         ach = top["alg_bytes_per_launch"] / (avg * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": top["name"], "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": NCU_TRAFFIC_CFG4.get(top["name"]) if args.cfg == 4 else None,
-                "traffic_source": "profiles/r1e_ncu_full_cfg4.md" if args.cfg == 4 else None, "peak_source": peak_src,
+                "frac": ach / peak, "traffic": NCU_TRAFFIC_CFG4.get(top["name"]) if full_cfg4 else None,
+                "traffic_source": "profiles/r1e_ncu_full_cfg4.md" if full_cfg4 else None, "peak_source": peak_src,
                 "alg_bytes_per_launch": top["alg_bytes_per_launch"], "avg_launch_ms": avg}
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
     if args.method == "rk4ip":
@@ -343,6 +344,8 @@ def main():
     ap.add_argument("--impl", default="mmf", choices=["mmf", "reference"])
     ap.add_argument("--method", default="rk4ip", choices=["rk4ip", "ssfm"],
                     help="rk4ip (Eq. 6, the headline path) or ssfm (SSFM-RK4, the symmetric split step of Eq. 4)")
+    ap.add_argument("--modes", type=int, default=None, help="override the config's mode count M (extra data points)")
+    ap.add_argument("--logn", type=int, default=None, help="override the config's N = 2^logn (extra data points)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT reference point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
