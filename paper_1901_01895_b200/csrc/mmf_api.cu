@@ -448,6 +448,7 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
   if (logn <= MMF_TILE_LOG) p->logn1 = 0;
   else if (logn == 13) p->logn1 = 6;
   else if (logn <= 15) p->logn1 = 8;
+  else if (logn <= 20) p->logn1 = 8;   // N2 <= 2^12; the 256-byte segments of W = 16 columns stream best
   else if (logn <= 22) p->logn1 = 10;
   else p->logn1 = 12;
   p->logn2 = logn - p->logn1;
