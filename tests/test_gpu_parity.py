@@ -220,3 +220,36 @@ def test_error_paths_on_device(mmf, torch):
     assert L.mmf_propagate(pl._h, None, 1, None) == mmf.MMF_EINVAL
     assert L.mmf_propagate(pl._h, ctypes.c_void_p(X.data_ptr() + 8), 1, None) == mmf.MMF_EINVAL
     assert L.mmf_plan_set_workspace(pl._h, ctypes.c_void_p(pl._ws_ptr), 16, None) == mmf.MMF_EINVAL
+
+
+# ------------------------------------------------------------------------------------------ parameter edge cases
+@pytest.mark.parametrize("K,logn", [(1, 12), (2, 13), (6, 13), (8, 12)])
+def test_linear_operator_any_number_of_beta_terms(mmf, torch, orc, K, logn):
+    """K Taylor coefficients beta_0..beta_{K-1}, all non-zero, per mode different (Eq. 1, reading R2)."""
+    M, N, dt, h, alpha = 3, 1 << logn, 0.5, 40.0, 3e-4
+    rng = np.random.default_rng(K * 100 + logn)
+    beta = rng.uniform(-1, 1, size=(M, K)) * (0.02 / (np.arange(K) + 1.0) ** 3)[None, :]
+    X = rand_c(rng, 2 * M, N)
+    X[:, N // 2] = 0
+    A = np.fft.ifft(X, axis=1)
+    pl = mmf.Plan(M, N, dt, h, alpha, beta, 0.0, np.eye(M))
+    D = to_dev(torch, A)
+    pl.apply_linear(D)
+    E = orc.linear_table(M, N, dt, h / 2, alpha, beta)
+    want = orc.apply_D(A, E)
+    assert workloads.rel_l2_per_field(D.cpu().numpy(), want).max() <= 5e-14
+
+
+def test_propagate_non_symmetric_kappa_no_loss_single_sample_tile(mmf, torch, orc):
+    """kappa not symmetric, alpha = 0, K = 3, M = 5 (ragged mode groups), N = 16 (the smallest transform)."""
+    M, N, dt, h, steps = 5, 16, 1.0, 0.5, 6
+    rng = np.random.default_rng(2024)
+    A = rand_c(rng, 2 * M, N) * 0.5
+    beta = rng.uniform(-0.05, 0.05, size=(M, 3))
+    kappa = rng.uniform(0.1, 1.0, size=(M, M))
+    pl = mmf.Plan(M, N, dt, h, 0.0, beta, 0.1, kappa)
+    X = to_dev(torch, A)
+    pl.propagate(X, steps)
+    want = orc.rk4ip(A, dt, h, 0.0, beta, 0.1, kappa, steps)
+    assert workloads.rel_l2_per_field(want, A).min() > 1e-3
+    assert workloads.rel_l2_per_field(X.cpu().numpy(), want).max() <= TOL_FIELD
