@@ -209,11 +209,7 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   constexpr size_t smem = cols_smem_bytes<LOGN1>();
   constexpr int LOGW = MMF_TILE_LOG - LOGN1;
   auto kern = k_cols<LOGN1, DIR, kGroups>;
-  static bool attr_done = false;
-  if (!attr_done) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_done = true;
-  }
+  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
   ColsParams q;
   q.twtab = p->d_tw1; q.ipt = p->d_ipt;
   q.logn2 = p->logn2; q.nrows = 2 * p->M; q.nbuf = nbuf;
@@ -246,11 +242,7 @@ int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   constexpr size_t smem = rows_smem_bytes<LOGN2>();
   constexpr int LOGB = MMF_TILE_LOG - LOGN2;
   auto kern = k_rows<LOGN2, MODE, SINGLE, kGroups>;
-  static bool attr_done = false;
-  if (!attr_done) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_done = true;
-  }
+  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
   RowsParams q;
   q.X0 = X0; q.X1 = X1; q.E = p->E; q.twtab = p->d_tw2;
   q.nchunks = (2LL * p->M) << p->logn1;
@@ -299,11 +291,7 @@ template <int MODE>
 int launch_nl(mmf_plan* p, cpx* X, cpx* Y, cpx* Z, cpx* W, cudaStream_t st) {
   auto kern = k_nl<MODE>;
   const size_t smem = nl_smem_bytes(p);
-  static size_t attr_smem = 0;
-  if (smem > attr_smem) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_smem = smem;
-  }
+  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
   NlParams q;
   q.X = X; q.Y = Y; q.Z = Z; q.W = W;
   q.kappa = p->d_kappa;
@@ -366,11 +354,7 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st) {
   if ((rc = field_tile_map(p, B, &mapB)) != MMF_OK) return rc;
   const size_t smem = nlt_smem_bytes(p->M, NK, NARR);
   const int threads = 32 * (q.NW + 1);
-  static size_t attr_smem = 0;
-  if (smem > attr_smem) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_smem = smem;
-  }
+  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
   int occ = 1;
   CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
   if (occ < 1) return MMF_EINVAL;
