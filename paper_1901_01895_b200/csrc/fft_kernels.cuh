@@ -58,8 +58,19 @@ __host__ __device__ constexpr int ipt_row_entries(int logw) { return 256 + (2 <<
 struct ColsParams {
   const cpx* __restrict__ twtab;  // stage tables of the N1-point transform
   const cpx* __restrict__ ipt;    // inter-pass table [N2 / W][256 + 2 W]
-  int logn2, nrows, nbuf;
+  int logn2, logwb, nrows, nbuf;
 };
+
+// BLOCKED field layout (the order every kernel between mmf_propagate's entry and exit works in when N > 4096).
+// A row of N = N1 N2 samples, n = N2 n1 + n2 with n2 = WB ctb + cb (WB = 2^logwb = max(W, 16) columns per block), is
+// stored as [ctb][n1][cb]: position (ctb N1 + n1) WB + cb.  Measured with a pure TMA copy: in the
+// natural order the tile of passes A / C (64-byte segments at 64 KiB pitch) streams at 4.7 TB/s and the contiguous
+// chunk of pass B at 6.3; in the blocked order the A / C tile (64-byte segments at 256-byte pitch inside one
+// contiguous block) streams at 5.2 TB/s and the chunk of pass B (256-byte segments) at 5.9 — and pass B, bound by
+// its arithmetic, needs only 3.7.  The nonlinear kernels act on every time sample alike and never see the
+// difference (8 consecutive positions are still 8 time samples, the same for every row).  k_perm converts a buffer
+// between the natural and the blocked order on the way in and out.
+__host__ __device__ constexpr int block_logw(int logn1) { return (MMF_TILE_LOG - logn1) > 4 ? (MMF_TILE_LOG - logn1) : 4; }
 
 // v[j] *= W_N^(k1(pos0 + j) n2)  (or its conjugate): the 16 factors are t0 sA^(j&7) sB^(j>>3) — three look-ups per
 // thread and short product chains (depth <= 4).
@@ -107,12 +118,12 @@ __host__ __device__ constexpr size_t cols_smem_bytes() {
 
 // grid = persistent (<= one CTA per SM); block = 512 = two groups of 256.  DIR 0: pass A (DIF, sign +, then twiddle);
 // DIR 1: pass C (conjugate twiddle, then DIT, sign -).  A tile is N1 points x W = 2^(12 - LOGN1) adjacent columns of
-// one field row, i.e. the box (2 W doubles, N1 rows) of the 2-D tensor map (inner = 2 N2 doubles, outer = rows x N1,
-// stride N2 complex) at (2 W ct, row N1), moved in boxes of <= 256 rows.
+// one field row: in the blocked layout the box (2 W doubles, N1 rows) at (2 W (ct % (WB/W)), (row N2/WB + ct / (WB/W)) N1)
+// of the 2-D tensor map (inner = 2 WB doubles, outer = rows x N2/WB x N1), moved in boxes of <= 256 rows.
 // Data movement is asynchronous and off the LSU pipe: the CTA's tiles t = 0, 1, 2, ... rotate through S ring slots
 // (slot t % S), tile t is worked on by group t % 2 IN its slot (the slot is also the group's exchange buffer), and the
-// group's first thread stores it with TMA and then refills the slot its previous tile vacated with tile t - 2 + S,
-// which the other group picks up half a tile period later.  map0 / map1: the two field buffers.
+// group's first thread stores it and then refills the slot its previous tile vacated with tile t - 2 + S, which the
+// other group picks up half a tile period later.  map0 / map1: the two field buffers.
 template <int LOGN1, int DIR, int G>
 __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1)
 k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, ColsParams p) {
@@ -153,13 +164,14 @@ k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
   const long long total = nct * p.nrows * p.nbuf;
   const long long ntile = total > blockIdx.x ? (total - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
 
-  // global coordinates of the CTA's tile tt, and its TMA traffic
+  // tensor-map coordinates of the CTA's tile tt (blocked layout), its buffer and its column tile
+  const int logsub = p.logwb - LOGW;  // column tiles per block
   auto tile_coords = [&](long long tt, int& c0, int& c1, const CUtensorMap*& m, long long& ct) {
     const long long u = blockIdx.x + tt * gridDim.x;
     ct = u & (nct - 1);
     const long long rb = u >> (logn2 - LOGW);
-    c0 = (int)(ct << (LOGW + 1));                       // doubles
-    c1 = (int)(rb % p.nrows) << LOGN1;                  // memory row of the (rows x N1, N2) view
+    c0 = (int)(ct & ((1 << logsub) - 1)) << (LOGW + 1);                                       // doubles
+    c1 = (int)((((rb % p.nrows) << (logn2 - p.logwb)) + (ct >> logsub)) << LOGN1);            // pitch row
     m = (rb / p.nrows) ? &map1 : &map0;
   };
   auto issue_load = [&](long long tt) {
@@ -236,14 +248,85 @@ k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
   if (elect) tma_store_wait_all();
 }
 
+// ---------------------------------------------------------------------------------------- natural <-> blocked order
+// A copy of the A / C tiles through a three-slot ring driven by one thread per CTA; DIR 0: natural -> blocked,
+// DIR 1: blocked -> natural.  mapn: the natural buffer as doubles [rows N1][2 N2]; mapb: the blocked buffer as
+// doubles [rows N2/WB N1][2 WB]; box of both = 2 W doubles x min(N1, 256) rows.  mmf_propagate runs it once on the
+// way in and once on the way out.  grid = persistent, block = 32.
+struct PermParams {
+  int logn2, logwb, nrows;
+};
+template <int LOGN1, int DIR>
+__global__ void __launch_bounds__(32, 1)
+k_perm(const __grid_constant__ CUtensorMap mapn, const __grid_constant__ CUtensorMap mapb, PermParams p) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  constexpr int LOGW = MMF_TILE_LOG - LOGN1, W = 1 << LOGW;
+  constexpr int S = 3;
+  constexpr int TILE_BYTES = (int)sizeof(cpx) << MMF_TILE_LOG;
+  constexpr int RB = LOGN1 > 8 ? 256 : (1 << LOGN1);  // rows per TMA box
+  constexpr int NBOX = (1 << LOGN1) / RB;
+  constexpr int BOX_BYTES = RB * W * (int)sizeof(cpx);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S * TILE_BYTES);
+  if (threadIdx.x != 0) return;
+#pragma unroll
+  for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
+  mbar_init_fence();
+  tma_prefetch_desc(&mapn);
+  tma_prefetch_desc(&mapb);
+  const int logn2 = p.logn2, logsub = p.logwb - LOGW;
+  const long long nct = 1LL << (logn2 - LOGW);
+  const long long total = nct * p.nrows;
+  const long long ntile = total > blockIdx.x ? (total - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  const CUtensorMap* src = DIR == 0 ? &mapn : &mapb;
+  const CUtensorMap* dst = DIR == 0 ? &mapb : &mapn;
+  // coordinates of tile tt in the natural (which = 0) or the blocked (which = 1) map
+  auto coords = [&](long long tt, int which, int& c0, int& c1) {
+    const long long u = blockIdx.x + tt * gridDim.x;
+    const long long ct = u & (nct - 1), row = u >> (logn2 - LOGW);
+    if (which == 0) {
+      c0 = (int)(ct << (LOGW + 1));
+      c1 = (int)row << LOGN1;
+    } else {
+      c0 = (int)(ct & ((1 << logsub) - 1)) << (LOGW + 1);
+      c1 = (int)(((row << (logn2 - p.logwb)) + (ct >> logsub)) << LOGN1);
+    }
+  };
+  auto load = [&](long long tt) {
+    int c0, c1;
+    coords(tt, DIR, c0, c1);
+    const int b = (int)(tt % S);
+    unsigned char* sl = smem_raw + (size_t)b * TILE_BYTES;
+    mbar_arrive_expect_tx(&full[b], TILE_BYTES);
+#pragma unroll
+    for (int i = 0; i < NBOX; ++i) tma_load_2d(sl + i * BOX_BYTES, src, c0, c1 + i * RB, &full[b]);
+  };
+  for (long long tt = 0; tt < S - 1 && tt < ntile; ++tt) load(tt);
+  for (long long tt = 0; tt < ntile; ++tt) {
+    const int b = (int)(tt % S);
+    if (tt + S - 1 < ntile) {  // the slot of tile tt - 1: refill it once its store has read it
+      if (tt >= 1) tma_store_wait_read();
+      load(tt + S - 1);
+    }
+    mbar_wait(&full[b], (uint32_t)((tt / S) & 1));
+    int c0, c1;
+    coords(tt, 1 - DIR, c0, c1);
+    const unsigned char* sl = smem_raw + (size_t)b * TILE_BYTES;
+#pragma unroll
+    for (int i = 0; i < NBOX; ++i) tma_store_2d(dst, c0, c1 + i * RB, sl + i * BOX_BYTES);
+    tma_store_commit();
+  }
+  tma_store_wait_all();
+}
+
 // -------------------------------------------------------------------------------------------------------- pass B
 // A "chunk" is one contiguous run of N2 values (memory row p1 of field row r: chunk = r * N1 + p1); a tile is
 // 2^(12 - LOGN2) consecutive chunks = 64 KiB of contiguous memory.  The exp(h/2 L) table holds, per (mode, p1) chunk,
 // its N2 entries in the register order of the last forward stage: entry [(q & 15) << (LOGN2 - 4) | (q >> 4)] belongs
 // to slot q, so that lanes read consecutive entries.
 struct RowsParams {
-  cpx* X0;
+  cpx* X0;                        // SINGLE: the field buffers (natural order); else unused (tensor maps)
   cpx* X1;
+  cpx* OUT;                       // MODE 1: where the slot-order spectrum goes (chunk-contiguous)
   const cpx* __restrict__ E;
   const cpx* __restrict__ twtab;  // stage tables of the N2-point transform
   long long nchunks;              // per buffer: 2 M N1
@@ -264,10 +347,14 @@ __host__ __device__ constexpr size_t rows_smem_bytes() {
 // j = 0, 1, ... (item blockIdx.x + j gridDim.x) go to group j % 2.
 // Data movement: as in k_cols — the CTA's tiles tt = 0, 1, ... (group tt % 2, sub-tile (tt / 2) % sub of item
 // 2 (tt / (2 sub)) + tt % 2) rotate through three 64 KiB ring slots that are also the exchange buffers; a tile is one
-// contiguous bulk copy each way (cp.async.bulk), issued by the group's first thread.  The sub-tiles of an odd last
-// item alternate between the groups, so the rotation has no holes.
+// bulk copy each way, issued by the group's first thread: contiguous (cp.async.bulk) when N <= 4096, else — blocked
+// layout — chunk p1 of a row is the box (2 WB doubles) x (N2 / WB rows) at (2 WB p1, row N2 / WB) of the 2-D tensor
+// map (inner = 2 N1 WB doubles = one block, outer = rows x N2 / WB), moved in boxes of <= 256 rows; the box lands as
+// [ctb][cb] = the chunk in n2 order.  The sub-tiles of an odd last item alternate between the groups, so the
+// rotation has no holes.  map0 / map1: the two field buffers (unused when SINGLE).
 template <int LOGN2, int MODE, bool SINGLE, int G>
-__global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) {
+__global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1)
+k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, RowsParams p) {
   static_assert(G == 2, "two groups alternate over the ring");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   constexpr int LOGB = MMF_TILE_LOG - LOGN2;
@@ -348,6 +435,20 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
       return TILE_BYTES;
     }
   };
+  // blocked layout: the boxes of one chunk (block width, boxes per chunk and rows per box depend on N1)
+  const int logwb = SINGLE ? 0 : block_logw(logn1);
+  const int lognb = LOGN2 - logwb;                                 // blocks (pitch rows) per chunk
+  auto chunk_boxes = [&](long long chunk, int buf, unsigned char* sl, uint64_t* bar) {
+    const CUtensorMap* m = buf ? &map1 : &map0;
+    const int rbr = lognb > 8 ? 256 : (1 << lognb), nboxc = (1 << lognb) / rbr;
+    const int box_bytes = (rbr << logwb) * (int)sizeof(cpx);
+    const int c0 = (int)(chunk & ((1LL << logn1) - 1)) << (logwb + 1);
+    const int c1 = (int)(chunk >> logn1) << lognb;
+    for (int i = 0; i < nboxc; ++i) {
+      if (bar) tma_load_2d(sl + i * box_bytes, m, c0, c1 + i * rbr, bar);
+      else tma_store_2d(m, c0, c1 + i * rbr, sl + i * box_bytes);
+    }
+  };
   auto issue_load = [&](long long tt) {
     long long chunk0, item;
     int buf;
@@ -355,7 +456,12 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
     const int b = (int)(tt % S);
     const uint32_t bytes = tile_bytes(chunk0);
     mbar_arrive_expect_tx(&full[b], bytes);
-    bulk_load_1d(smem_raw + (size_t)b * TILE_BYTES, (buf ? p.X1 : p.X0) + (chunk0 << LOGN2), bytes, &full[b]);
+    if constexpr (SINGLE) {
+      bulk_load_1d(smem_raw + (size_t)b * TILE_BYTES, (buf ? p.X1 : p.X0) + (chunk0 << LOGN2), bytes, &full[b]);
+    } else {
+      for (int q = 0; q < (1 << LOGB); ++q)
+        chunk_boxes(chunk0 + q, buf, smem_raw + (size_t)b * TILE_BYTES + ((size_t)q << LOGN2) * sizeof(cpx), &full[b]);
+    }
     if constexpr (!SINGLE && MODE == 0) {
       // first sub-tile of an item (polarisation x of buffer 0): pull the item's piece of the table into L2
       if (buf == 0 && ((chunk0 >> logn1) & 1) == 0) {
@@ -365,8 +471,13 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
     }
   };
 
-  if (threadIdx.x == 0)
+  if (threadIdx.x == 0) {
+    if constexpr (!SINGLE) {
+      tma_prefetch_desc(&map0);
+      tma_prefetch_desc(&map1);
+    }
     for (long long tt = 0; tt < S && tt < ntile; ++tt) issue_load(tt);
+  }
 
   // Only the tile number stays live across the transforms: geometry is recomputed where it is needed (the table
   // pointer after the forward chain, the store address by the first thread) to keep the 16 values in registers.
@@ -436,7 +547,12 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
         int buf;
         tile_geom(tt, chunk0, buf, item);
         mbar_wait(&done[grp], (uint32_t)((tt >> 1) & 1));
-        bulk_store_1d((buf ? p.X1 : p.X0) + (chunk0 << LOGN2), s, tile_bytes(chunk0));
+        if constexpr (SINGLE) {
+          bulk_store_1d((buf ? p.X1 : p.X0) + (chunk0 << LOGN2), s, tile_bytes(chunk0));
+        } else {
+          for (int q = 0; q < (1 << LOGB); ++q)
+            chunk_boxes(chunk0 + q, buf, reinterpret_cast<unsigned char*>(s + ((size_t)q << LOGN2)), nullptr);
+        }
         tma_store_commit();
       }
     } else {
@@ -444,7 +560,7 @@ __global__ void __launch_bounds__(MMF_GROUP_THREADS* G, 1) k_rows(RowsParams p) 
       int buf;
       tile_geom(tt, chunk0, buf, item);
       if (!SINGLE || chunk0 + cht < p.nchunks) {
-        cpx* g = (buf ? p.X1 : p.X0) + (chunk0 << LOGN2);
+        cpx* g = p.OUT + (chunk0 << LOGN2);
 #pragma unroll
         for (int j = 0; j < 16; ++j) g[(t << 4) + j] = v[j];
       }

@@ -118,7 +118,7 @@ struct mmf_plan {
   dd* d_coefs = nullptr;
   unsigned char* ws = nullptr;
   size_t ws_bytes = 0, field_bytes = 0;
-  cpx *Y = nullptr, *Z = nullptr, *W = nullptr, *E = nullptr;
+  cpx *Y = nullptr, *Z = nullptr, *W = nullptr, *V = nullptr, *E = nullptr;
   long long launches = 0;
   // optional per-launch CUDA-event timing (mmf_plan_set_timing): one (start, stop) pair per launch
   bool timing = false;
@@ -131,10 +131,10 @@ namespace {
 
 // ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
 enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
-       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_COUNT };
+       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_PERM, KC_COUNT };
 const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
                                         "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>", "k_nlm<plain>",
-                                        "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>"};
+                                        "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>", "k_perm"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
 struct LaunchTimer {
@@ -180,18 +180,17 @@ EncodeTiledFn encode_tiled_fn() {
   return fn;
 }
 
-// tensor map of a field buffer for passes A / C: the buffer seen as doubles [2M N1][2 N2] (memory rows of N2 complex
-// values), box = (2 W doubles = W adjacent columns) x min(N1, 256) rows
-int cols_tile_map(const mmf_plan* p, const void* base, int logn1, CUtensorMap* map) {
+// 2-D tensor map of a field buffer seen as doubles [nrows_outer][2 * inner complex], box = (2 W doubles) x boxrows
+int strided_tile_map(const void* base, cuuint64_t inner_cpx, cuuint64_t nrows_outer, int logw, cuuint32_t boxrows,
+                     CUtensorMap* map) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) {
     snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled is unavailable");
     return MMF_ECUDA;
   }
-  const int logw = MMF_TILE_LOG - logn1;
-  const cuuint64_t gdim[2] = {(cuuint64_t)2 << p->logn2, ((cuuint64_t)(2 * p->M)) << logn1};
-  const cuuint64_t gstride[1] = {sizeof(cpx) << p->logn2};
-  const cuuint32_t box[2] = {(cuuint32_t)2 << logw, (cuuint32_t)(logn1 > 8 ? 256 : (1 << logn1))};
+  const cuuint64_t gdim[2] = {2 * inner_cpx, nrows_outer};
+  const cuuint64_t gstride[1] = {sizeof(cpx) * inner_cpx};
+  const cuuint32_t box[2] = {(cuuint32_t)2 << logw, boxrows};
   const cuuint32_t estr[2] = {1, 1};
   const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), gdim, gstride, box, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
@@ -203,6 +202,30 @@ int cols_tile_map(const mmf_plan* p, const void* base, int logn1, CUtensorMap* m
   return MMF_OK;
 }
 
+// NATURAL order, the column tile of passes A / C (used by k_perm): memory rows of N2 complex values, rows x N1 of them;
+// box = W adjacent columns x min(N1, 256) rows
+int natural_cols_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+  const int logw = MMF_TILE_LOG - p->logn1;
+  return strided_tile_map(base, 1ULL << p->logn2, ((cuuint64_t)(2 * p->M)) << p->logn1, logw,
+                          p->logn1 > 8 ? 256u : (1u << p->logn1), map);
+}
+
+// BLOCKED order (fft_kernels.cuh), the column tile of passes A / C: pitch rows of WB complex values, rows x N2/WB x N1
+// of them; box = W adjacent columns x min(N1, 256) rows
+int blocked_cols_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+  const int logw = MMF_TILE_LOG - p->logn1, logwb = block_logw(p->logn1);
+  return strided_tile_map(base, 1ULL << logwb, ((cuuint64_t)(2 * p->M)) << (p->logn2 - logwb + p->logn1), logw,
+                          p->logn1 > 8 ? 256u : (1u << p->logn1), map);
+}
+
+// BLOCKED order, the chunk of pass B: pitch rows of one block (N1 WB complex values), rows x N2/WB of them;
+// box = the WB values of one (block, p1) x min(N2/WB, 256) blocks
+int blocked_rows_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+  const int logwb = block_logw(p->logn1), lognb = p->logn2 - logwb;
+  return strided_tile_map(base, 1ULL << (p->logn1 + logwb), ((cuuint64_t)(2 * p->M)) << lognb, logwb,
+                          lognb > 8 ? 256u : (1u << lognb), map);
+}
+
 // ---- launch helpers ----------------------------------------------------------------------------------------------
 template <int LOGN1, int DIR>
 int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
@@ -212,11 +235,11 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
   ColsParams q;
   q.twtab = p->d_tw1; q.ipt = p->d_ipt;
-  q.logn2 = p->logn2; q.nrows = 2 * p->M; q.nbuf = nbuf;
+  q.logn2 = p->logn2; q.logwb = block_logw(LOGN1); q.nrows = 2 * p->M; q.nbuf = nbuf;
   CUtensorMap map0, map1;
   int rc;
-  if ((rc = cols_tile_map(p, X0, LOGN1, &map0)) != MMF_OK) return rc;
-  if ((rc = cols_tile_map(p, nbuf > 1 ? X1 : X0, LOGN1, &map1)) != MMF_OK) return rc;
+  if ((rc = blocked_cols_map(p, X0, &map0)) != MMF_OK) return rc;
+  if ((rc = blocked_cols_map(p, nbuf > 1 ? X1 : X0, &map1)) != MMF_OK) return rc;
   const long long tiles = ((long long)nbuf * 2 * p->M) << (p->logn2 - LOGW);
   long long grid = tiles < p->num_sms ? tiles : p->num_sms;
   LaunchTimer lt(p, DIR == 0 ? KC_COLS_FWD : KC_COLS_INV, 2 * nbuf, st);
@@ -237,30 +260,39 @@ int launch_cols(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   }
 }
 
+// X0 / X1: the field buffers (tiled order unless SINGLE); OUT: MODE 1 only, receives the slot-order spectrum
 template <int LOGN2, int MODE, bool SINGLE>
-int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
+int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cpx* OUT, cudaStream_t st) {
   constexpr size_t smem = rows_smem_bytes<LOGN2>();
   constexpr int LOGB = MMF_TILE_LOG - LOGN2;
   auto kern = k_rows<LOGN2, MODE, SINGLE, kGroups>;
   CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
   RowsParams q;
-  q.X0 = X0; q.X1 = X1; q.E = p->E; q.twtab = p->d_tw2;
+  q.X0 = X0; q.X1 = nbuf > 1 ? X1 : X0; q.OUT = OUT; q.E = p->E; q.twtab = p->d_tw2;
+  CUtensorMap map0, map1;
+  memset(&map0, 0, sizeof(map0));
+  memset(&map1, 0, sizeof(map1));
+  if (!SINGLE) {
+    int rc;
+    if ((rc = blocked_rows_map(p, q.X0, &map0)) != MMF_OK) return rc;
+    if ((rc = blocked_rows_map(p, q.X1, &map1)) != MMF_OK) return rc;
+  }
   q.nchunks = (2LL * p->M) << p->logn1;
   q.logn1 = p->logn1; q.nbuf = nbuf; q.M = p->M;
   const long long items = SINGLE ? ((q.nchunks + (1 << LOGB) - 1) >> LOGB) : ((long long)p->M << (p->logn1 - LOGB));
   long long grid = items < p->num_sms ? items : p->num_sms;
   LaunchTimer lt(p, KC_ROWS, 2 * nbuf, st);
-  kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(q);
+  kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(map0, map1, q);
   p->launches++;
   CU(cudaGetLastError());
   return MMF_OK;
 }
 
 template <int MODE>
-int launch_rows(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
+int launch_rows(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cpx* OUT, cudaStream_t st) {
   if (p->logn1 == 0) {
     switch (p->logn2) {
-#define MMF_ROWS_CASE(L) case L: return launch_rows_t<L, MODE, true>(p, X0, X1, nbuf, st);
+#define MMF_ROWS_CASE(L) case L: return launch_rows_t<L, MODE, true>(p, X0, X1, nbuf, OUT, st);
       MMF_ROWS_CASE(4) MMF_ROWS_CASE(5) MMF_ROWS_CASE(6) MMF_ROWS_CASE(7) MMF_ROWS_CASE(8) MMF_ROWS_CASE(9)
       MMF_ROWS_CASE(10) MMF_ROWS_CASE(11) MMF_ROWS_CASE(12)
 #undef MMF_ROWS_CASE
@@ -268,7 +300,7 @@ int launch_rows(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
     }
   }
   switch (p->logn2) {
-#define MMF_ROWS_CASE(L) case L: return launch_rows_t<L, MODE, false>(p, X0, X1, nbuf, st);
+#define MMF_ROWS_CASE(L) case L: return launch_rows_t<L, MODE, false>(p, X0, X1, nbuf, OUT, st);
     MMF_ROWS_CASE(6) MMF_ROWS_CASE(7) MMF_ROWS_CASE(8) MMF_ROWS_CASE(9) MMF_ROWS_CASE(10) MMF_ROWS_CASE(11)
     MMF_ROWS_CASE(12)
 #undef MMF_ROWS_CASE
@@ -276,14 +308,49 @@ int launch_rows(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   }
 }
 
-// D on one or two full-field buffers: exp(h/2 L) in place (rows a1-a3 of the hot path).
+// D on one or two full-field buffers: exp(h/2 L) in place (rows a1-a3 of the hot path).  For N > 4096 the buffers are
+// in the BLOCKED order (fft_kernels.cuh); to_tiled / to_natural convert on the way in and out of a propagation.
 int apply_D(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   int rc;
   if (p->logn1 > 0 && (rc = launch_cols<0>(p, X0, X1, nbuf, st)) != MMF_OK) return rc;
-  if ((rc = launch_rows<0>(p, X0, X1, nbuf, st)) != MMF_OK) return rc;
+  if ((rc = launch_rows<0>(p, X0, X1, nbuf, nullptr, st)) != MMF_OK) return rc;
   if (p->logn1 > 0 && (rc = launch_cols<1>(p, X0, X1, nbuf, st)) != MMF_OK) return rc;
   return MMF_OK;
 }
+
+// DIR 0: tiled <- natural (out of place);  DIR 1: natural <- tiled.  Only for N > 4096 (logn1 > 0).
+template <int LOGN1, int DIR>
+int launch_perm_t(mmf_plan* p, cpx* natural, cpx* tiled, cudaStream_t st) {
+  constexpr size_t smem = 3 * (sizeof(cpx) << MMF_TILE_LOG) + 64;
+  constexpr int LOGW = MMF_TILE_LOG - LOGN1;
+  auto kern = k_perm<LOGN1, DIR>;
+  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  CUtensorMap mapn, mapb;
+  int rc;
+  if ((rc = natural_cols_map(p, natural, &mapn)) != MMF_OK) return rc;
+  if ((rc = blocked_cols_map(p, tiled, &mapb)) != MMF_OK) return rc;
+  PermParams q;
+  q.logn2 = p->logn2; q.logwb = block_logw(LOGN1); q.nrows = 2 * p->M;
+  const long long tiles = ((long long)2 * p->M) << (p->logn2 - LOGW);
+  long long grid = tiles < p->num_sms ? tiles : p->num_sms;
+  LaunchTimer lt(p, KC_PERM, 2, st);
+  kern<<<(unsigned)grid, 32, smem, st>>>(mapn, mapb, q);
+  p->launches++;
+  CU(cudaGetLastError());
+  return MMF_OK;
+}
+template <int DIR>
+int launch_perm(mmf_plan* p, cpx* natural, cpx* tiled, cudaStream_t st) {
+  switch (p->logn1) {
+    case 6: return launch_perm_t<6, DIR>(p, natural, tiled, st);
+    case 8: return launch_perm_t<8, DIR>(p, natural, tiled, st);
+    case 10: return launch_perm_t<10, DIR>(p, natural, tiled, st);
+    case 12: return launch_perm_t<12, DIR>(p, natural, tiled, st);
+    default: return MMF_EINVAL;
+  }
+}
+int to_tiled(mmf_plan* p, cpx* natural, cpx* tiled, cudaStream_t st) { return launch_perm<0>(p, natural, tiled, st); }
+int to_natural(mmf_plan* p, cpx* tiled, cpx* natural, cudaStream_t st) { return launch_perm<1>(p, natural, tiled, st); }
 
 size_t nl_smem_bytes(const mmf_plan* p) { return sizeof(double) * 2 * (size_t)p->M * MMF_NL_T; }
 
@@ -505,7 +572,8 @@ size_t mmf_plan_workspace_bytes(const mmf_plan* p) {
   if (!p) return 0;
   const size_t F = align_up(p->field_bytes, 256);
   const size_t E = align_up(sizeof(cpx) * (size_t)p->M * (size_t)p->N, 256);
-  return (p->nlm_nk > 0 ? 1 : 3) * F + E;
+  // tensor-path plan: one more field buffer; DFMA plan (M > 120): three, plus one to hold the field in tiled order
+  return (p->nlm_nk > 0 ? 1 : (p->logn1 > 0 ? 4 : 3)) * F + E;
 }
 
 int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_stream) {
@@ -517,12 +585,13 @@ int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_s
   p->ws_bytes = bytes;
   p->Y = (cpx*)(p->ws);
   if (p->nlm_nk > 0) {
-    p->Z = p->W = nullptr;
+    p->Z = p->W = p->V = nullptr;
     p->E = (cpx*)(p->ws + F);
   } else {
     p->Z = (cpx*)(p->ws + F);
     p->W = (cpx*)(p->ws + 2 * F);
-    p->E = (cpx*)(p->ws + 3 * F);
+    p->V = p->logn1 > 0 ? (cpx*)(p->ws + 3 * F) : nullptr;
+    p->E = (cpx*)(p->ws + (p->logn1 > 0 ? 4 : 3) * F);
   }
   EtabParams P;
   memset(&P, 0, sizeof(P));
@@ -545,10 +614,19 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   if (!p->ws) return MMF_EINVAL;
   if (nsteps == 0) return MMF_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  cpx *X = (cpx*)A_dev, *Y = p->Y, *Z = p->Z, *W = p->W;
+  cpx* A = (cpx*)A_dev;
+  const bool tiled = p->logn1 > 0;  // N > 4096: every kernel below works in the blocked order (fft_kernels.cuh)
   int rc;
   if (p->nlm_nk > 0) {
-    // two full-field buffers: X (the caller's field) and Y.  Per step: D(X,Y); S23 in place; D(X,Y); FINAL(+NEXT).
+    // two full-field buffers: the caller's and Y.  The field X moves to Y on its way into the tiled order and the
+    // caller's buffer serves as the second buffer; the way back to the natural order brings it home.
+    cpx *X = A, *Y = p->Y;
+    if (tiled) {
+      if ((rc = to_tiled(p, A, p->Y, st)) != MMF_OK) return rc;
+      X = p->Y;
+      Y = A;
+    }
+    // per step: D(X,Y); S23 in place; D(X,Y); FINAL(+NEXT)
     if ((rc = launch_nlm<NLM_PLAIN>(p, X, Y, st)) != MMF_OK) return rc;   // Y <- h N(A) A   (6b bracket)
     for (int s = 0; s < nsteps; ++s) {
       if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6a) A_I, (6b) k1
@@ -558,7 +636,13 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
       else rc = launch_nlm<NLM_FINAL>(p, X, Y, st);
       if (rc != MMF_OK) return rc;
     }
+    if (tiled && (rc = to_natural(p, X, A, st)) != MMF_OK) return rc;
     return MMF_OK;
+  }
+  cpx *X = A, *Y = p->Y, *Z = p->Z, *W = p->W;
+  if (tiled) {
+    if ((rc = to_tiled(p, A, p->V, st)) != MMF_OK) return rc;
+    X = p->V;
   }
   // the bracket of Eq. (6b) for the first step; later steps get it from NL_FINAL_NEXT
   if ((rc = launch_nl<NL_PLAIN>(p, X, Y, Z, W, st)) != MMF_OK) return rc;
@@ -571,20 +655,28 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
     else rc = launch_nl<NL_FINAL>(p, X, Y, Z, W, st);
     if (rc != MMF_OK) return rc;
   }
+  if (tiled && (rc = to_natural(p, X, A, st)) != MMF_OK) return rc;
   return MMF_OK;
 }
 
 int mmf_propagate_ssfm(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   if (!p || !A_dev || nsteps < 0 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
   if (!p->ws || p->nlm_nk <= 0) return MMF_EINVAL;  // the fused RK4 substep exists on the tensor path only (M <= 120)
+  if (nsteps == 0) return MMF_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  cpx* X = (cpx*)A_dev;
+  cpx *A = (cpx*)A_dev, *X = A;
+  const bool tiled = p->logn1 > 0;
   int rc;
+  if (tiled) {
+    if ((rc = to_tiled(p, A, p->Y, st)) != MMF_OK) return rc;
+    X = p->Y;
+  }
   for (int s = 0; s < nsteps; ++s) {
     if ((rc = apply_D(p, X, X, 1, st)) != MMF_OK) return rc;              // exp(h/2 L)
     if ((rc = launch_nlm<NLM_RK4>(p, X, X, st)) != MMF_OK) return rc;     // RK4 over h of dA/dz = N(A) A
     if ((rc = apply_D(p, X, X, 1, st)) != MMF_OK) return rc;              // exp(h/2 L)
   }
+  if (tiled && (rc = to_natural(p, X, A, st)) != MMF_OK) return rc;
   return MMF_OK;
 }
 
@@ -601,7 +693,13 @@ int mmf_propagate_host(mmf_plan* p, void* A_host, void* A_dev_scratch, int nstep
 
 int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
   if (!p || !X_dev || !p->ws || ((size_t)X_dev & 15) != 0) return MMF_EINVAL;
-  return apply_D(p, (cpx*)X_dev, (cpx*)X_dev, 1, (cudaStream_t)cuda_stream);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cpx* X = (cpx*)X_dev;
+  if (p->logn1 == 0) return apply_D(p, X, X, 1, st);
+  int rc;  // N > 4096: through the tiled order, with the workspace's field buffer as the working copy
+  if ((rc = to_tiled(p, X, p->Y, st)) != MMF_OK) return rc;
+  if ((rc = apply_D(p, p->Y, p->Y, 1, st)) != MMF_OK) return rc;
+  return to_natural(p, p->Y, X, st);
 }
 
 int mmf_apply_nonlinear(mmf_plan* p, const void* U_dev, void* OUT_dev, void* cuda_stream) {
@@ -614,8 +712,15 @@ int mmf_debug_forward(mmf_plan* p, void* X_dev, void* SPEC_dev, void* cuda_strea
   if (!p || !X_dev || !SPEC_dev || X_dev == SPEC_dev) return MMF_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc;
-  if (p->logn1 > 0 && (rc = launch_cols<0>(p, (cpx*)X_dev, (cpx*)X_dev, 1, st)) != MMF_OK) return rc;
-  if ((rc = launch_rows<1>(p, (cpx*)X_dev, (cpx*)X_dev, 1, st)) != MMF_OK) return rc;
+  cpx *X = (cpx*)X_dev, *S = (cpx*)SPEC_dev;
+  if (p->logn1 > 0) {
+    // SPEC holds the working copy in tiled order; pass B leaves the slot-order spectrum in X (chunk-contiguous)
+    if ((rc = to_tiled(p, X, S, st)) != MMF_OK) return rc;
+    if ((rc = launch_cols<0>(p, S, S, 1, st)) != MMF_OK) return rc;
+    if ((rc = launch_rows<1>(p, S, S, 1, X, st)) != MMF_OK) return rc;
+  } else {
+    if ((rc = launch_rows<1>(p, X, X, 1, X, st)) != MMF_OK) return rc;
+  }
   dim3 grid((unsigned)((p->N + 255) / 256), (unsigned)(2 * p->M));
   k_unpermute<<<grid, 256, 0, st>>>((const cpx*)X_dev, (cpx*)SPEC_dev, p->logn1, p->logn2);
   p->launches++;
