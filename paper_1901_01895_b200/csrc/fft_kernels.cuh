@@ -249,56 +249,48 @@ k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
 }
 
 // ---------------------------------------------------------------------------------------- natural <-> blocked order
-// A copy of the A / C tiles through a three-slot ring driven by one thread per CTA; DIR 0: natural -> blocked,
-// DIR 1: blocked -> natural.  mapn: the natural buffer as doubles [rows N1][2 N2]; mapb: the blocked buffer as
-// doubles [rows N2/WB N1][2 WB]; box of both = 2 W doubles x min(N1, 256) rows.  mmf_propagate runs it once on the
-// way in and once on the way out.  grid = persistent, block = 32.
+// A copy through a three-slot ring driven by one thread per CTA; DIR 0: natural -> blocked, DIR 1: blocked ->
+// natural.  A tile is RT = 4096 / WB consecutive memory rows n1 of one block: in the natural buffer the box
+// (2 WB doubles = 256-byte segments, RT rows) of the map (inner = 2 N2 doubles, outer = rows x N1), in the blocked
+// buffer 64 KiB of contiguous memory.  mmf_propagate runs it once on the way in and once on the way out.
+// grid = persistent, block = 32.
 struct PermParams {
-  int logn2, logwb, nrows;
+  cpx* blocked;
+  int logn1, logn2, logwb, nrows;
 };
-template <int LOGN1, int DIR>
-__global__ void __launch_bounds__(32, 1)
-k_perm(const __grid_constant__ CUtensorMap mapn, const __grid_constant__ CUtensorMap mapb, PermParams p) {
+template <int DIR>
+__global__ void __launch_bounds__(32, 1) k_perm(const __grid_constant__ CUtensorMap mapn, PermParams p) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
-  constexpr int LOGW = MMF_TILE_LOG - LOGN1, W = 1 << LOGW;
   constexpr int S = 3;
   constexpr int TILE_BYTES = (int)sizeof(cpx) << MMF_TILE_LOG;
-  constexpr int RB = LOGN1 > 8 ? 256 : (1 << LOGN1);  // rows per TMA box
-  constexpr int NBOX = (1 << LOGN1) / RB;
-  constexpr int BOX_BYTES = RB * W * (int)sizeof(cpx);
   uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S * TILE_BYTES);
   if (threadIdx.x != 0) return;
 #pragma unroll
   for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
   mbar_init_fence();
   tma_prefetch_desc(&mapn);
-  tma_prefetch_desc(&mapb);
-  const int logn2 = p.logn2, logsub = p.logwb - LOGW;
-  const long long nct = 1LL << (logn2 - LOGW);
-  const long long total = nct * p.nrows;
+  const int logrt = MMF_TILE_LOG - p.logwb;                 // rows per tile
+  const int lognb = p.logn2 - p.logwb;                      // blocks per row
+  const int logtb = p.logn1 - logrt;                        // tiles per block
+  const long long total = (long long)p.nrows << (lognb + logtb);
   const long long ntile = total > blockIdx.x ? (total - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
-  const CUtensorMap* src = DIR == 0 ? &mapn : &mapb;
-  const CUtensorMap* dst = DIR == 0 ? &mapb : &mapn;
-  // coordinates of tile tt in the natural (which = 0) or the blocked (which = 1) map
-  auto coords = [&](long long tt, int which, int& c0, int& c1) {
+  // tile u = (row, block ctb, row group i): natural box coordinates and blocked address
+  auto coords = [&](long long tt, int& c0, int& c1, cpx*& g) {
     const long long u = blockIdx.x + tt * gridDim.x;
-    const long long ct = u & (nct - 1), row = u >> (logn2 - LOGW);
-    if (which == 0) {
-      c0 = (int)(ct << (LOGW + 1));
-      c1 = (int)row << LOGN1;
-    } else {
-      c0 = (int)(ct & ((1 << logsub) - 1)) << (LOGW + 1);
-      c1 = (int)(((row << (logn2 - p.logwb)) + (ct >> logsub)) << LOGN1);
-    }
+    const long long ctb = u & ((1LL << lognb) - 1), i = (u >> lognb) & ((1LL << logtb) - 1), row = u >> (lognb + logtb);
+    c0 = (int)(ctb << (p.logwb + 1));
+    c1 = (int)((row << p.logn1) + (i << logrt));
+    g = p.blocked + ((((row << lognb) + ctb) << p.logn1) << p.logwb) + (i << MMF_TILE_LOG);
   };
   auto load = [&](long long tt) {
     int c0, c1;
-    coords(tt, DIR, c0, c1);
+    cpx* g;
+    coords(tt, c0, c1, g);
     const int b = (int)(tt % S);
     unsigned char* sl = smem_raw + (size_t)b * TILE_BYTES;
     mbar_arrive_expect_tx(&full[b], TILE_BYTES);
-#pragma unroll
-    for (int i = 0; i < NBOX; ++i) tma_load_2d(sl + i * BOX_BYTES, src, c0, c1 + i * RB, &full[b]);
+    if constexpr (DIR == 0) tma_load_2d(sl, &mapn, c0, c1, &full[b]);
+    else bulk_load_1d(sl, g, TILE_BYTES, &full[b]);
   };
   for (long long tt = 0; tt < S - 1 && tt < ntile; ++tt) load(tt);
   for (long long tt = 0; tt < ntile; ++tt) {
@@ -309,10 +301,11 @@ k_perm(const __grid_constant__ CUtensorMap mapn, const __grid_constant__ CUtenso
     }
     mbar_wait(&full[b], (uint32_t)((tt / S) & 1));
     int c0, c1;
-    coords(tt, 1 - DIR, c0, c1);
+    cpx* g;
+    coords(tt, c0, c1, g);
     const unsigned char* sl = smem_raw + (size_t)b * TILE_BYTES;
-#pragma unroll
-    for (int i = 0; i < NBOX; ++i) tma_store_2d(dst, c0, c1 + i * RB, sl + i * BOX_BYTES);
+    if constexpr (DIR == 0) bulk_store_1d(g, sl, TILE_BYTES);
+    else tma_store_2d(&mapn, c0, c1, sl);
     tma_store_commit();
   }
   tma_store_wait_all();

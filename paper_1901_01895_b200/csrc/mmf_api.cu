@@ -202,14 +202,6 @@ int strided_tile_map(const void* base, cuuint64_t inner_cpx, cuuint64_t nrows_ou
   return MMF_OK;
 }
 
-// NATURAL order, the column tile of passes A / C (used by k_perm): memory rows of N2 complex values, rows x N1 of them;
-// box = W adjacent columns x min(N1, 256) rows
-int natural_cols_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
-  const int logw = MMF_TILE_LOG - p->logn1;
-  return strided_tile_map(base, 1ULL << p->logn2, ((cuuint64_t)(2 * p->M)) << p->logn1, logw,
-                          p->logn1 > 8 ? 256u : (1u << p->logn1), map);
-}
-
 // BLOCKED order (fft_kernels.cuh), the column tile of passes A / C: pitch rows of WB complex values, rows x N2/WB x N1
 // of them; box = W adjacent columns x min(N1, 256) rows
 int blocked_cols_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
@@ -318,36 +310,27 @@ int apply_D(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   return MMF_OK;
 }
 
-// DIR 0: tiled <- natural (out of place);  DIR 1: natural <- tiled.  Only for N > 4096 (logn1 > 0).
-template <int LOGN1, int DIR>
-int launch_perm_t(mmf_plan* p, cpx* natural, cpx* tiled, cudaStream_t st) {
+// DIR 0: blocked <- natural (out of place);  DIR 1: natural <- blocked.  Only for N > 4096 (logn1 > 0).
+template <int DIR>
+int launch_perm(mmf_plan* p, cpx* natural, cpx* blocked, cudaStream_t st) {
   constexpr size_t smem = 3 * (sizeof(cpx) << MMF_TILE_LOG) + 64;
-  constexpr int LOGW = MMF_TILE_LOG - LOGN1;
-  auto kern = k_perm<LOGN1, DIR>;
+  auto kern = k_perm<DIR>;
   CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  CUtensorMap mapn, mapb;
+  const int logwb = block_logw(p->logn1);
+  CUtensorMap mapn;  // natural order: memory rows of N2 values, box = one block's WB columns x 4096 / WB rows
   int rc;
-  if ((rc = natural_cols_map(p, natural, &mapn)) != MMF_OK) return rc;
-  if ((rc = blocked_cols_map(p, tiled, &mapb)) != MMF_OK) return rc;
+  if ((rc = strided_tile_map(natural, 1ULL << p->logn2, ((cuuint64_t)(2 * p->M)) << p->logn1, logwb,
+                             1u << (MMF_TILE_LOG - logwb), &mapn)) != MMF_OK)
+    return rc;
   PermParams q;
-  q.logn2 = p->logn2; q.logwb = block_logw(LOGN1); q.nrows = 2 * p->M;
-  const long long tiles = ((long long)2 * p->M) << (p->logn2 - LOGW);
+  q.blocked = blocked; q.logn1 = p->logn1; q.logn2 = p->logn2; q.logwb = logwb; q.nrows = 2 * p->M;
+  const long long tiles = ((long long)2 * p->M) << (p->logn1 + p->logn2 - MMF_TILE_LOG);
   long long grid = tiles < p->num_sms ? tiles : p->num_sms;
   LaunchTimer lt(p, KC_PERM, 2, st);
-  kern<<<(unsigned)grid, 32, smem, st>>>(mapn, mapb, q);
+  kern<<<(unsigned)grid, 32, smem, st>>>(mapn, q);
   p->launches++;
   CU(cudaGetLastError());
   return MMF_OK;
-}
-template <int DIR>
-int launch_perm(mmf_plan* p, cpx* natural, cpx* tiled, cudaStream_t st) {
-  switch (p->logn1) {
-    case 6: return launch_perm_t<6, DIR>(p, natural, tiled, st);
-    case 8: return launch_perm_t<8, DIR>(p, natural, tiled, st);
-    case 10: return launch_perm_t<10, DIR>(p, natural, tiled, st);
-    case 12: return launch_perm_t<12, DIR>(p, natural, tiled, st);
-    default: return MMF_EINVAL;
-  }
 }
 int to_tiled(mmf_plan* p, cpx* natural, cpx* tiled, cudaStream_t st) { return launch_perm<0>(p, natural, tiled, st); }
 int to_natural(mmf_plan* p, cpx* tiled, cpx* natural, cudaStream_t st) { return launch_perm<1>(p, natural, tiled, st); }
