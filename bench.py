@@ -281,6 +281,8 @@ def run_mmf(args):
         balg = (14 if p.N > 4096 else 6) * F
     t_roof_ms = balg / (peak * 1e9) * 1e3
     step_roof = {"B_alg_bytes_per_step": balg, "hbm_time_ms": t_roof_ms, "frac": t_roof_ms / (ms / args.steps)}
+    if args.method == "rk4ip" and p.N > 4096:      # this plan's own count: (6c)+(6d) in one pass -> 32 F
+        step_roof["frac_of_32F_plan"] = (32 * F / (peak * 1e9) * 1e3) / (ms / args.steps)
 
     # ---- cuFFT (through torch.fft) beside the hand-written transforms: a reference point only, never on the path ----
     cufft = None
