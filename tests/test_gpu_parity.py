@@ -149,6 +149,7 @@ CASES = [
     (0, 2, 12, 100),      # config 0 at full size and step count
     (1, 6, 13, 40),
     (1, 6, 16, 12),       # config 1 at full size, shortened
+    (1, 6, 16, 250),      # config 1 at full size, a quarter of its 1000 steps: rounding errors stay far below the bar
     (2, 36, 14, 8),
     (3, 120, 13, 4),
     (4, 120, 14, 3),
