@@ -45,11 +45,11 @@ typedef struct mmf_plan mmf_plan; /* opaque */
 int mmf_plan_create(mmf_plan **out, int M, long long N, double dt, double h, double alpha, const double *beta, int K,
                     double gamma, const double *kappa);
 
-/* Bytes of device workspace the plan needs: one more full-field buffer (three when M > 120, four when also N > 4096)
- * plus the tabulated exp(h/2 L_a(w_k)) of Eq. (6a) (one row per mode).  The caller allocates it (e.g. a torch uint8
- * tensor), 256-byte aligned, and keeps it alive while the plan is used.  Note: for N > 4096 the library keeps the
- * field in an internal (blocked) sample order between the entry and the exit of mmf_propagate / mmf_propagate_ssfm /
- * mmf_apply_linear; A_dev is in the natural order documented above on entry and on return. */
+/* Bytes of device workspace the plan needs: one more full-field buffer when N <= 4096, two when N > 4096 (three resp.
+ * four when M > 120) plus the tabulated exp(h/2 L_a(w_k)) of Eq. (6a) (one row per mode).  The caller allocates it
+ * (e.g. a torch uint8 tensor), 256-byte aligned, and keeps it alive while the plan is used.  Note: for N > 4096 the
+ * library works on copies in an internal (blocked) sample order; A_dev is read in the natural order documented above
+ * by the first kernel of a call and written in it by the last one. */
 size_t mmf_plan_workspace_bytes(const mmf_plan *plan);
 
 /* Attach the workspace and fill the plan's tables in it (enqueues kernels on `cuda_stream`, a cudaStream_t passed

@@ -131,10 +131,11 @@ namespace {
 
 // ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
 enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
-       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_PERM, KC_COUNT };
+       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_NLM_ENTER, KC_NLM_EXIT, KC_PERM, KC_COUNT };
 const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
                                         "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>", "k_nlm<plain>",
-                                        "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>", "k_perm"};
+                                        "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>", "k_nlm<enter>",
+                                        "k_nlm<exit>", "k_perm"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
 struct LaunchTimer {
@@ -387,9 +388,10 @@ int field_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
   return MMF_OK;
 }
 
-// PLAIN: A = U, B = OUT; other modes: A = X, B = Y.
+// PLAIN: A = U, B = OUT; ENTER: A = the caller's field (natural order), B = X, C = Y; EXIT: A = X, B = Y, C = the
+// caller's field; other modes: A = X, B = Y (C unused).
 template <int NK, int MODE>
-int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st) {
+int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st) {
   auto kern = k_nlt<NK, MODE>;
   constexpr int NARR = nlm_narr<MODE>();
   NltParams q;
@@ -398,10 +400,12 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st) {
   q.M = p->M;
   q.NW = (p->M + 7) / 8;
   q.ntiles = p->N / MMF_NLM_T;
-  CUtensorMap mapA, mapB;
+  q.logn1 = p->logn1; q.logn2 = p->logn2; q.logwb = block_logw(p->logn1);
+  CUtensorMap mapA, mapB, mapC;
   int rc;
   if ((rc = field_tile_map(p, A, &mapA)) != MMF_OK) return rc;
   if ((rc = field_tile_map(p, B, &mapB)) != MMF_OK) return rc;
+  if ((rc = field_tile_map(p, C ? C : B, &mapC)) != MMF_OK) return rc;
   const size_t smem = nlt_smem_bytes(p->M, NK, NARR);
   const int threads = 32 * (q.NW + 1);
   CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
@@ -410,17 +414,17 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st) {
   if (occ < 1) return MMF_EINVAL;
   long long grid = (long long)p->num_sms * occ;        // persistent: every resident CTA walks its own tile list
   if (grid > q.ntiles) grid = q.ntiles;
-  LaunchTimer lt(p, KC_NLM_PLAIN + MODE, (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 2 : MODE == NLM_FINAL ? 3 : 4, st);
-  kern<<<(unsigned)grid, threads, smem, st>>>(mapA, mapB, q);
+  LaunchTimer lt(p, KC_NLM_PLAIN + MODE, (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 2 : (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT) ? 4 : 3, st);
+  kern<<<(unsigned)grid, threads, smem, st>>>(mapA, mapB, mapC, q);
   p->launches++;
   CU(cudaGetLastError());
   return MMF_OK;
 }
 
 template <int MODE>
-int launch_nlm(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st) {
+int launch_nlm(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st, cpx* C = nullptr) {
   switch (p->nlm_nk) {
-#define MMF_NLM_CASE(NKV) case NKV: return launch_nlm_t<NKV, MODE>(p, A, B, st);
+#define MMF_NLM_CASE(NKV) case NKV: return launch_nlm_t<NKV, MODE>(p, A, B, C, st);
     MMF_NLM_CASE(1) MMF_NLM_CASE(2) MMF_NLM_CASE(3) MMF_NLM_CASE(4) MMF_NLM_CASE(6) MMF_NLM_CASE(8) MMF_NLM_CASE(9)
     MMF_NLM_CASE(12) MMF_NLM_CASE(16) MMF_NLM_CASE(20) MMF_NLM_CASE(24) MMF_NLM_CASE(28) MMF_NLM_CASE(30)
     MMF_NLM_CASE(32)
@@ -556,7 +560,8 @@ size_t mmf_plan_workspace_bytes(const mmf_plan* p) {
   const size_t F = align_up(p->field_bytes, 256);
   const size_t E = align_up(sizeof(cpx) * (size_t)p->M * (size_t)p->N, 256);
   // tensor-path plan: one more field buffer; DFMA plan (M > 120): three, plus one to hold the field in tiled order
-  return (p->nlm_nk > 0 ? 1 : (p->logn1 > 0 ? 4 : 3)) * F + E;
+  // (N > 4096, tensor path: two, the field and the second buffer both live in the workspace in blocked order)
+  return (p->nlm_nk > 0 ? (p->logn1 > 0 ? 2 : 1) : (p->logn1 > 0 ? 4 : 3)) * F + E;
 }
 
 int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_stream) {
@@ -568,8 +573,9 @@ int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_s
   p->ws_bytes = bytes;
   p->Y = (cpx*)(p->ws);
   if (p->nlm_nk > 0) {
-    p->Z = p->W = p->V = nullptr;
-    p->E = (cpx*)(p->ws + F);
+    p->W = p->V = nullptr;
+    p->Z = p->logn1 > 0 ? (cpx*)(p->ws + F) : nullptr;  // second blocked-order buffer
+    p->E = (cpx*)(p->ws + (p->logn1 > 0 ? 2 : 1) * F);
   } else {
     p->Z = (cpx*)(p->ws + F);
     p->W = (cpx*)(p->ws + 2 * F);
@@ -601,25 +607,23 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   const bool tiled = p->logn1 > 0;  // N > 4096: every kernel below works in the blocked order (fft_kernels.cuh)
   int rc;
   if (p->nlm_nk > 0) {
-    // two full-field buffers: the caller's and Y.  The field X moves to Y on its way into the tiled order and the
-    // caller's buffer serves as the second buffer; the way back to the natural order brings it home.
-    cpx *X = A, *Y = p->Y;
-    if (tiled) {
-      if ((rc = to_tiled(p, A, p->Y, st)) != MMF_OK) return rc;
-      X = p->Y;
-      Y = A;
-    }
+    // two full-field buffers X, Y.  N <= 4096: the caller's buffer and the workspace's.  N > 4096: both in the
+    // workspace, in blocked order; the first and the last nonlinear kernel read / write the caller's buffer in its
+    // natural order, so the layout conversions cost no pass of their own.
+    cpx *X = tiled ? p->Y : A, *Y = tiled ? p->Z : p->Y;
     // per step: D(X,Y); S23 in place; D(X,Y); FINAL(+NEXT)
-    if ((rc = launch_nlm<NLM_PLAIN>(p, X, Y, st)) != MMF_OK) return rc;   // Y <- h N(A) A   (6b bracket)
+    if (tiled) rc = launch_nlm<NLM_ENTER>(p, A, X, st, Y);               // X <- A, Y <- h N(A) A   (6b bracket)
+    else rc = launch_nlm<NLM_PLAIN>(p, X, Y, st);
+    if (rc != MMF_OK) return rc;
     for (int s = 0; s < nsteps; ++s) {
       if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6a) A_I, (6b) k1
       if ((rc = launch_nlm<NLM_S23>(p, X, Y, st)) != MMF_OK) return rc;    // (6c), (6d), brackets of 6e/6f
       if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6e) argument, (6f) first term
       if (s + 1 < nsteps) rc = launch_nlm<NLM_FINAL_NEXT>(p, X, Y, st);    // (6e)+(6f), next (6b) bracket
+      else if (tiled) rc = launch_nlm<NLM_EXIT>(p, X, Y, st, A);           // (6e)+(6f) into the caller's buffer
       else rc = launch_nlm<NLM_FINAL>(p, X, Y, st);
       if (rc != MMF_OK) return rc;
     }
-    if (tiled && (rc = to_natural(p, X, A, st)) != MMF_OK) return rc;
     return MMF_OK;
   }
   cpx *X = A, *Y = p->Y, *Z = p->Z, *W = p->W;

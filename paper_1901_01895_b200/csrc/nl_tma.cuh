@@ -9,6 +9,12 @@
 //               instead of the 8 F two kernels need.
 //   NLM_FINAL   X = u4, Y = exp(h/2 L)[...]:  X <- Y + NL(X)/6                   (Eq. 6e + 6f; Y untouched)
 //   NLM_FINAL_NEXT  as NLM_FINAL, then Y <- NL(X_new)                           (the next step's Eq. 6b bracket)
+//   NLM_ENTER   first kernel of a propagation in the blocked order (fft_kernels.cuh): reads tile tn(t) of the caller's
+//               field A (NATURAL order) and writes tile t of X <- A and of Y <- NL(A) (blocked order): the layout
+//               conversion of the way in rides on the first nonlinear evaluation (3 F instead of 2 F + 2 F).
+//   NLM_EXIT    last kernel: NLM_FINAL on the blocked X, Y with the result written to tile tn(t) of the caller's
+//               field (natural order): no conversion pass on the way out.
+//               A time tile is 8 consecutive samples in both orders; only its position differs.
 //   NLM_RK4     X <- X + k1/6 + k2/3 + k3/3 + k4/6,  k1 = NL(X), k2 = NL(X + k1/2), k3 = NL(X + k2/2), k4 = NL(X + k3):
 //               the nonlinear substep of the symmetric split step (Eq. 4, "SSFM-RK4"): classical RK4
 //               over h of dA/dz = N(A) A, four contraction rounds per tile, the field read and written once (2 F).
@@ -30,7 +36,7 @@
 
 namespace mmf {
 
-enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3, NLM_RK4 = 4 };
+enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3, NLM_RK4 = 4, NLM_ENTER = 5, NLM_EXIT = 6 };
 
 #define MMF_NLM_T 8           // time samples per tile
 #define MMF_NLM_PSTRIDE 12    // doubles per P row in shared memory (8 + 4: conflict-free B-fragment reads)
@@ -42,6 +48,7 @@ struct NltParams {
   double hg;
   int M;
   int NW;            // compute warps = ceil(M / 8); the producer is warp NW
+  int logn1, logn2, logwb;  // NLM_ENTER / NLM_EXIT: geometry of the blocked order (N = N1 N2, WB columns per block)
   long long ntiles;  // N / 8
 };
 
@@ -52,7 +59,7 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 }
 
 template <int MODE>
-__host__ __device__ constexpr int nlm_narr() { return (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 1 : 2; }
+__host__ __device__ constexpr int nlm_narr() { return (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 1 : 2; }  // arrays per slot
 
 // bytes of dynamic shared memory: ring slots, two P buffers, mbarriers
 __host__ __device__ inline size_t nlt_slot_bytes(int M, int narr) { return (size_t)narr * 2 * M * MMF_NLM_T * sizeof(cpx); }
@@ -82,7 +89,8 @@ __device__ __forceinline__ cpx axpy(double s, cpx a, cpx b) { return make_double
 // block = 32 (NW + 1) threads; grid = persistent; dynamic smem = nlt_smem_bytes(M, NK, narr).
 template <int NK, int MODE>
 __global__ void __launch_bounds__(512, 1)
-k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, NltParams p) {
+k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
+      const __grid_constant__ CUtensorMap mapC, NltParams p) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   constexpr int NARR = nlm_narr<MODE>();
   constexpr bool TWO_ROUNDS = (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT);
@@ -113,14 +121,29 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
     if (lane != 0) return;
     tma_prefetch_desc(&mapA);
     tma_prefetch_desc(&mapB);
-    const CUtensorMap* out0 = (MODE == NLM_PLAIN) ? &mapB : &mapA;
+    tma_prefetch_desc(&mapC);
+    // natural-order tile that holds the samples of blocked tile t (ENTER reads it, EXIT writes it)
+    auto natural_tile = [&](long long t) -> long long {
+      const int u8 = p.logwb - 3;  // log2(tiles per unit of WB columns)
+      const long long cbt = t & ((1LL << u8) - 1), unit = t >> u8;
+      const long long n1 = unit & ((1LL << p.logn1) - 1), ctb = unit >> p.logn1;
+      return (n1 << (p.logn2 - 3)) + (ctb << u8) + cbt;
+    };
     auto store_tile = [&](long long tl, int slot) {
       unsigned char* s = smem_raw + slot * slot_bytes;
-      tma_store_2d(out0, (int)(tl * 2 * MMF_NLM_T), 0, s);
-      if constexpr (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT)
-        tma_store_2d(&mapB, (int)(tl * 2 * MMF_NLM_T), 0, s + arr_elems * sizeof(cpx));
+      const int c0 = (int)(tl * 2 * MMF_NLM_T);
+      if constexpr (MODE == NLM_ENTER) {  // X <- A and Y <- NL(A), blocked order
+        tma_store_2d(&mapB, c0, 0, s);
+        tma_store_2d(&mapC, c0, 0, s + arr_elems * sizeof(cpx));
+      } else if constexpr (MODE == NLM_EXIT) {  // the new field, natural order
+        tma_store_2d(&mapC, (int)(natural_tile(tl) * 2 * MMF_NLM_T), 0, s);
+      } else {
+        tma_store_2d((MODE == NLM_PLAIN) ? &mapB : &mapA, c0, 0, s);
+        if constexpr (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT) tma_store_2d(&mapB, c0, 0, s + arr_elems * sizeof(cpx));
+      }
       tma_store_commit();
     };
+    constexpr uint32_t kLoadArrays = (MODE == NLM_ENTER) ? 1 : NARR;
     long long tile = blockIdx.x;
     int j = 0;
     for (; tile < p.ntiles; tile += tstep, ++j) {
@@ -131,9 +154,10 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
         store_tile(tile - MMF_NLM_SLOTS * tstep, slot);
         tma_store_wait_read();
       }
-      mbar_arrive_expect_tx(&full[slot], (uint32_t)slot_bytes);
-      tma_load_2d(s, &mapA, (int)(tile * 2 * MMF_NLM_T), 0, &full[slot]);
-      if constexpr (NARR == 2) tma_load_2d(s + arr_elems * sizeof(cpx), &mapB, (int)(tile * 2 * MMF_NLM_T), 0, &full[slot]);
+      mbar_arrive_expect_tx(&full[slot], (uint32_t)(kLoadArrays * arr_elems * sizeof(cpx)));
+      const long long tin = (MODE == NLM_ENTER) ? natural_tile(tile) : tile;
+      tma_load_2d(s, &mapA, (int)(tin * 2 * MMF_NLM_T), 0, &full[slot]);
+      if constexpr (kLoadArrays == 2) tma_load_2d(s + arr_elems * sizeof(cpx), &mapB, (int)(tile * 2 * MMF_NLM_T), 0, &full[slot]);
     }
     for (int jj = (j > MMF_NLM_SLOTS ? j - MMF_NLM_SLOTS : 0); jj < j; ++jj) {  // drain
       const int slot = jj % MMF_NLM_SLOTS, use = jj / MMF_NLM_SLOTS;
@@ -174,7 +198,7 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
 #pragma unroll
       for (int i = 0; i < 2; ++i) {
         x[pol][i] = valid ? sx[e0 + pol * MMF_NLM_T + i] : make_double2(0.0, 0.0);
-        if constexpr (NARR == 2) y[pol][i] = valid ? sy[e0 + pol * MMF_NLM_T + i] : make_double2(0.0, 0.0);
+        if constexpr (NARR == 2 && MODE != NLM_ENTER) y[pol][i] = valid ? sy[e0 + pol * MMF_NLM_T + i] : make_double2(0.0, 0.0);
         if constexpr (MODE == NLM_S23) u[pol][i] = axpy(0.5, y[pol][i], x[pol][i]);
         else u[pol][i] = x[pol][i];
       }
@@ -220,14 +244,15 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
     nlm_contract<NK>(kf, P1, g, q, s[0], s[1]);
     const double g1[2] = {p.hg * s[0], p.hg * s[1]};
 
-    if constexpr (MODE == NLM_PLAIN) {
+    if constexpr (MODE == NLM_PLAIN || MODE == NLM_ENTER) {
+      cpx* so = (MODE == NLM_ENTER) ? sy : sx;  // ENTER keeps the field in the first array of the slot
       if (valid) {
 #pragma unroll
         for (int pol = 0; pol < 2; ++pol)
 #pragma unroll
-          for (int i = 0; i < 2; ++i) sx[e0 + pol * MMF_NLM_T + i] = times_ig(u[pol][i], g1[i]);
+          for (int i = 0; i < 2; ++i) so[e0 + pol * MMF_NLM_T + i] = times_ig(u[pol][i], g1[i]);
       }
-    } else if constexpr (MODE == NLM_FINAL) {
+    } else if constexpr (MODE == NLM_FINAL || MODE == NLM_EXIT) {
       if (valid) {
 #pragma unroll
         for (int pol = 0; pol < 2; ++pol)
