@@ -33,7 +33,7 @@ def log(*a):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the committed `ncu --set full` capture of this
-# command on cfg4 (profiles/r1g_ncu_full_cfg4.md); other workloads have no capture: traffic = null.
+# command on cfg4 (profiles/r1h_ncu_full_cfg4.md); other workloads have no capture: traffic = null.
 NCU_TRAFFIC_CFG4 = {"k_rows": 74.32e9, "k_cols<fwd>": 65.62e9, "k_cols<inv>": 65.47e9, "k_nlm<s23>": 64.38e9,
                     "k_nlm<final_next>": 64.36e9}
 
@@ -272,7 +272,7 @@ def run_mmf(args):
         ach = top["alg_bytes_per_launch"] / (avg * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": top["name"], "achieved": ach, "peak": peak, "unit": "GB/s",
                 "frac": ach / peak, "traffic": NCU_TRAFFIC_CFG4.get(top["name"]) if full_cfg4 else None,
-                "traffic_source": "profiles/r1g_ncu_full_cfg4.md" if full_cfg4 else None, "peak_source": peak_src,
+                "traffic_source": "profiles/r1h_ncu_full_cfg4.md" if full_cfg4 else None, "peak_source": peak_src,
                 "alg_bytes_per_launch": top["alg_bytes_per_launch"], "avg_launch_ms": avg}
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
     if args.method == "rk4ip":
