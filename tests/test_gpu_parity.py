@@ -155,6 +155,7 @@ CASES = [
     (4, 120, 14, 3),
     (4, 7, 18, 3),        # config-4 physics at the 2^18 transform size, odd mode count
     (3, 124, 13, 2),      # more than 120 modes: the DFMA nonlinear kernels and the four-buffer plan
+    (4, 1, 23, 1),        # N = 2^23: N1 = 2^12, one-column tiles (W = 1) inside 16-column blocks
 ]
 
 
