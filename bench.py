@@ -274,6 +274,15 @@ def run_mmf(args):
                 "frac": ach / peak, "traffic": NCU_TRAFFIC_CFG4.get(top["name"]) if full_cfg4 else None,
                 "traffic_source": "profiles/r1h_ncu_full_cfg4.md" if full_cfg4 else None, "peak_source": peak_src,
                 "alg_bytes_per_launch": top["alg_bytes_per_launch"], "avg_launch_ms": avg}
+        if full_cfg4 and top["name"] == "k_rows":
+            # second bound of the same kernel: fp64 issue.  Thread-level fp64 instructions of one launch from the
+            # committed ncu capture (smsp__inst_executed x fp64 share, profiles/r1h_ncu_full_cfg4.md); peak = 64 per
+            # clock per SM x 148 SMs (measured with a DADD / DMUL stream) at the clock seen under load.
+            fp64_inst = 1.69e11
+            clk = (clocks.get("sm_mhz") or 1965.0) * 1e6
+            peak_i = 64.0 * 148 * clk
+            roof["fp64_issue"] = {"achieved_Tinst_s": fp64_inst / (avg * 1e-3) / 1e12, "peak_Tinst_s": peak_i / 1e12,
+                                  "frac": fp64_inst / (avg * 1e-3) / peak_i, "sm_mhz": clk / 1e6}
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
     if args.method == "rk4ip":
         balg = (36 if p.N > 4096 else 20) * F
