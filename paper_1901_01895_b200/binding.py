@@ -17,7 +17,8 @@ MMF_OK, MMF_EINVAL, MMF_ENOMEM, MMF_ECUDA = 0, -1, -2, -3
 SYMBOLS = ["mmf_plan_create", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate", "mmf_propagate_ssfm",
            "mmf_propagate_host", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
            "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_set_timing", "mmf_kernel_class_count",
-           "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version"]
+           "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version",
+           "mmf_probe_fp64", "mmf_probe_tma_copy"]
 
 _lib = None
 
@@ -71,6 +72,11 @@ def lib():
     L.mmf_plan_destroy.restype = i
     L.mmf_status_string.argtypes = [i]
     L.mmf_status_string.restype = ctypes.c_char_p
+    ull, u = ctypes.c_ulonglong, ctypes.c_uint
+    L.mmf_probe_fp64.argtypes = [i, i, i, dp, dp]
+    L.mmf_probe_fp64.restype = i
+    L.mmf_probe_tma_copy.argtypes = [vp, sz, ull, ull, ull, u, u, i, i, i, i, ll, i, i, i, dp, dp]
+    L.mmf_probe_tma_copy.restype = i
     L.mmf_version.argtypes = []
     L.mmf_version.restype = ctypes.c_char_p
     _lib = L
@@ -198,3 +204,21 @@ def raw_create(M, N, dt, h, alpha, beta, K, gamma, kappa):
     rc = lib().mmf_plan_create(ctypes.byref(h_), int(M), int(N), float(dt), float(h), float(alpha), b, int(K),
                                float(gamma), k)
     return rc, h_
+
+
+def probe_fp64(kind, threads=512, iters=4000):
+    """mmf_probe_fp64: (ms per launch, thread-level (kind 5: warp-level) instructions per launch)."""
+    ms, n = ctypes.c_double(), ctypes.c_double()
+    _check(lib().mmf_probe_fp64(int(kind), int(threads), int(iters), ctypes.byref(ms), ctypes.byref(n)), "mmf_probe_fp64")
+    return ms.value, n.value
+
+
+def probe_tma_copy(buf, dim0, dim1, stride_bytes, box0, box1, nbox, nct_log, c0_mul, c1_mul, ntiles, slots=3, bulk=0,
+                   reps=3):
+    """mmf_probe_tma_copy over the torch uint8 CUDA tensor `buf`: (ms per launch, bytes moved read + write)."""
+    ms, by = ctypes.c_double(), ctypes.c_double()
+    _check(lib().mmf_probe_tma_copy(ctypes.c_void_p(buf.data_ptr()), buf.numel(), int(dim0), int(dim1), int(stride_bytes),
+                                    int(box0), int(box1), int(nbox), int(nct_log), int(c0_mul), int(c1_mul), int(ntiles),
+                                    int(slots), int(bulk), int(reps), ctypes.byref(ms), ctypes.byref(by)),
+           "mmf_probe_tma_copy")
+    return ms.value, by.value

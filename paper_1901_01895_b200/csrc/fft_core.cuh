@@ -6,9 +6,9 @@
 //   * a "tile" is 2^12 complex values worked on by one GROUP of 256 threads; every thread owns 16 values
 //     (64 registers) and performs radix-2..16 butterflies on them;
 //   * a transform of 2^LOGP points is split into NST = ceil(LOGP/4) digits.  The FIRST stage takes its 16 values
-//     straight from global memory and the LAST stage leaves them in registers for the epilogue (spectral multiply,
-//     inter-pass twiddle, store): shared memory is only the exchange buffer BETWEEN stages (one STS.128 + one
-//     LDS.128 per value per exchange, one group barrier per exchange);
+//     from the tile TMA staged in shared memory and the LAST stage leaves them in registers for the epilogue
+//     (spectral multiply, inter-pass twiddle); the same shared-memory slot is the exchange buffer BETWEEN stages
+//     (one STS.128 + one LDS.128 per value per exchange, one group barrier per exchange);
 //   * decimation in frequency on the way to the spectrum, the exact adjoint (decimation in time) on the way back,
 //     so no bit-reversal pass exists: the spectrum stays in digit-reversed slot order, the last forward stage and
 //     the first inverse stage share one register layout, and the exp(h/2 L) table is stored in that order;

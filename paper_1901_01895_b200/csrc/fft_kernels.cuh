@@ -13,9 +13,9 @@
 //
 // Execution model: persistent CTAs (one per SM) of G independent groups of 256 threads.  A group owns one 64 KiB
 // exchange buffer and walks its own list of 4096-point tiles (fft_core.cuh); groups of a CTA share the stage
-// twiddle tables in shared memory and run out of phase, so that one group's global loads overlap the other's
-// butterflies.  Global loads go straight into the registers of the first stage and the last stage stores from
-// registers.
+// twiddle tables in shared memory and run out of phase, so that one group's exchanges overlap the other's
+// butterflies.  Tiles travel between HBM and shared memory as TMA bulk copies through a three-slot ring (the slot is
+// also the group's exchange buffer); no compute warp issues a global load or store.
 #pragma once
 #include "async_copy.cuh"
 #include "fft_core.cuh"
@@ -35,9 +35,6 @@ __host__ __device__ inline int slot_to_bin_rt(int logn, int p) {
   }
   return k;
 }
-
-__device__ __forceinline__ cpx ld_stream(const cpx* p) { return __ldcs(p); }
-__device__ __forceinline__ void st_stream(cpx* p, cpx v) { __stcs(p, v); }
 
 // copy the stage tables of a transform into shared memory (whole CTA), then synchronise
 template <int ENTRIES>
@@ -374,7 +371,10 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
     mbar_init_fence();
   }
   if constexpr (ECACHE) {
-    if (threadIdx.x < 32) tmem_alloc(tmem_word, TMEM_COLS);
+    if (threadIdx.x < 32) {
+      __syncwarp();  // reconverge after the single-thread block above: tcgen05.alloc is .sync.aligned
+      tmem_alloc(tmem_word, TMEM_COLS);
+    }
     tmem_fence_before_sync();
   }
   load_stage_tables<TWN>(tab, p.twtab);  // ends with __syncthreads

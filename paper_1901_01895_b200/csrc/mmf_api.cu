@@ -1,5 +1,6 @@
 // mmf_api.cu — the C ABI of include/mmf.h: plan management, table generation and the per-step launch sequence.
-// The product path: every step of the hot path runs in the kernels of kernels.cuh; there is no CPU fallback.
+// The product path: every step of the hot path runs in the kernels of fft_kernels.cuh / nl_tma.cuh / nl_simt.cuh;
+// there is no CPU fallback.
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -110,6 +111,7 @@ struct mmf_plan {
   int M = 0, K = 0, logn = 0, logn1 = 0, logn2 = 0;
   int nlm_nk = -1;   // k-steps of the tensor-path nonlinear kernel; -1: M too large, legacy kernels (4 buffers)
   int num_sms = 148;
+  int device = 0;    // the device the plan's tables live on; every call must be made with it current
   long long N = 0;
   double dt = 0, h = 0, alpha = 0, gamma = 0;
   std::vector<double> beta, kappa;
@@ -433,6 +435,12 @@ int launch_nlm(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st, cpx* C = null
   }
 }
 
+// a plan's tables, workspace and tensor maps belong to one device: refuse calls made with another one current
+bool on_plan_device(const mmf_plan* p) {
+  int dev = -1;
+  return cudaGetDevice(&dev) == cudaSuccess && dev == p->device;
+}
+
 bool finite_all(const double* v, size_t n) {
   for (size_t i = 0; i < n; ++i)
     if (!std::isfinite(v[i])) return false;
@@ -493,9 +501,8 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
   p->nlm_nk = (M <= MMF_NLM_MAXM) ? nlm_pick_nk(M) : -1;
   {
     int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
-      p->num_sms = sms;
+    if (cudaGetDevice(&dev) == cudaSuccess) p->device = dev;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) p->num_sms = sms;
   }
   p->field_bytes = sizeof(cpx) * 2 * (size_t)M * (size_t)N;
   int rc = MMF_OK;
@@ -565,7 +572,7 @@ size_t mmf_plan_workspace_bytes(const mmf_plan* p) {
 }
 
 int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_stream) {
-  if (!p || !ws_dev) return MMF_EINVAL;
+  if (!p || !ws_dev || !on_plan_device(p)) return MMF_EINVAL;
   if (bytes < mmf_plan_workspace_bytes(p) || ((size_t)ws_dev & 255) != 0) return MMF_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t F = align_up(p->field_bytes, 256);
@@ -600,7 +607,7 @@ int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_s
 
 int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   if (!p || !A_dev || nsteps < 0 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
-  if (!p->ws) return MMF_EINVAL;
+  if (!p->ws || !on_plan_device(p)) return MMF_EINVAL;
   if (nsteps == 0) return MMF_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cpx* A = (cpx*)A_dev;
@@ -648,7 +655,7 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
 
 int mmf_propagate_ssfm(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
   if (!p || !A_dev || nsteps < 0 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
-  if (!p->ws || p->nlm_nk <= 0) return MMF_EINVAL;  // the fused RK4 substep exists on the tensor path only (M <= 120)
+  if (!p->ws || p->nlm_nk <= 0 || !on_plan_device(p)) return MMF_EINVAL;  // the fused RK4 substep exists on the tensor path only (M <= 120)
   if (nsteps == 0) return MMF_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cpx *A = (cpx*)A_dev, *X = A;
@@ -679,7 +686,7 @@ int mmf_propagate_host(mmf_plan* p, void* A_host, void* A_dev_scratch, int nstep
 }
 
 int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
-  if (!p || !X_dev || !p->ws || ((size_t)X_dev & 15) != 0) return MMF_EINVAL;
+  if (!p || !X_dev || !p->ws || ((size_t)X_dev & 15) != 0 || !on_plan_device(p)) return MMF_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cpx* X = (cpx*)X_dev;
   if (p->logn1 == 0) return apply_D(p, X, X, 1, st);
@@ -690,13 +697,13 @@ int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
 }
 
 int mmf_apply_nonlinear(mmf_plan* p, const void* U_dev, void* OUT_dev, void* cuda_stream) {
-  if (!p || !U_dev || !OUT_dev || (((size_t)U_dev | (size_t)OUT_dev) & 15) != 0) return MMF_EINVAL;
+  if (!p || !U_dev || !OUT_dev || (((size_t)U_dev | (size_t)OUT_dev) & 15) != 0 || !on_plan_device(p)) return MMF_EINVAL;
   if (p->nlm_nk > 0) return launch_nlm<NLM_PLAIN>(p, (const cpx*)U_dev, (cpx*)OUT_dev, (cudaStream_t)cuda_stream);
   return launch_nl<NL_PLAIN>(p, (cpx*)U_dev, (cpx*)OUT_dev, nullptr, nullptr, (cudaStream_t)cuda_stream);
 }
 
 int mmf_debug_forward(mmf_plan* p, void* X_dev, void* SPEC_dev, void* cuda_stream) {
-  if (!p || !X_dev || !SPEC_dev || X_dev == SPEC_dev) return MMF_EINVAL;
+  if (!p || !X_dev || !SPEC_dev || X_dev == SPEC_dev || !on_plan_device(p)) return MMF_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc;
   cpx *X = (cpx*)X_dev, *S = (cpx*)SPEC_dev;
@@ -716,7 +723,7 @@ int mmf_debug_forward(mmf_plan* p, void* X_dev, void* SPEC_dev, void* cuda_strea
 }
 
 int mmf_debug_freq_index(mmf_plan* p, long long* idx_host) {
-  if (!p || !idx_host) return MMF_EINVAL;
+  if (!p || !idx_host || !on_plan_device(p)) return MMF_EINVAL;
   long long* d = nullptr;
   CU(cudaMalloc((void**)&d, sizeof(long long) * (size_t)p->N));
   k_slot_map<<<(unsigned)((p->N + 255) / 256), 256>>>(d, p->logn1, p->logn2);

@@ -18,7 +18,7 @@ def mmf():
 
 def test_library_exports_every_declared_symbol(mmf):
     hdr = open(os.path.join(ROOT, "include", "mmf.h")).read()
-    declared = set(re.findall(r"\b(mmf_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(mmf_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(mmf.SYMBOLS), declared ^ set(mmf.SYMBOLS)
     L = mmf.lib()
     for s in declared:

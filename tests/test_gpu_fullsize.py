@@ -177,3 +177,88 @@ def test_cfg4_full_step_energy(mmf, torch, orc, cfg4):
     d_orc = float(np.sum(np.abs(Bs) ** 2) / np.sum(np.abs(As) ** 2)) / math.exp(-ps.alpha * ps.h) - 1.0
     assert abs(d_gpu) <= 1e-6 and abs(d_orc) <= 1e-6
     assert abs(d_gpu - d_orc) <= 0.05 * abs(d_orc) + 1e-10, (d_gpu, d_orc)
+
+
+# ------------------------------------------- the timed plan, FULL physics, EVERY element, all 50 steps (north_star)
+# A field whose 2^22 samples are one 2^14-sample block repeated 256 times is periodic with the block length: its
+# spectrum lives on the bins k = 256 j only, and those carry exactly the block problem's frequencies
+# (w_k = 2 pi 256 j / (2^22 dt) = 2 pi j / (2^14 dt), same dt; k >= N/2 <=> j >= N_s/2, so the negative-frequency fold
+# and the Nyquist bin agree too).  D maps periodic fields to periodic fields, N acts sample by sample, so every stage
+# of Eq. (6) keeps the period and the exact result is the 256-fold tiling of the oracle's result on the 240 x 2^14
+# block — full physics (alpha, beta_1..3, gamma, the 120 x 120 kappa), every kernel of the timed configuration at
+# full size (all tiles, both buffers, ENTER / S23 / FINAL_NEXT / EXIT), all 50 steps, every element compared.
+TILE_LOGN = 14
+
+
+def tiled_cfg4(torch, scale=1.0):
+    p = workloads.problem(4)
+    ps = workloads.problem(4, N=1 << TILE_LOGN)
+    small = field_threaded(ps) * scale
+    X = torch.from_numpy(small).to("cuda:0").repeat(1, p.N >> TILE_LOGN).contiguous()
+    return p, ps, small, X
+
+
+def tiled_error(torch, X, want_small):
+    """per-field relative L2 of the whole X [R][reps * Ns] against the tiling of want_small [R][Ns], and max |diff|"""
+    R, Ns = want_small.shape
+    W = torch.from_numpy(want_small).to(X.device)
+    Xv = X.view(R, -1, Ns)
+    num = torch.empty(R, dtype=torch.float64, device=X.device)
+    dmax = 0.0
+    for r0 in range(0, R, 8):
+        d = torch.view_as_real(Xv[r0:r0 + 8] - W[r0:r0 + 8, None, :])
+        num[r0:r0 + 8] = (d * d).sum(dim=(1, 2, 3))
+        dmax = max(dmax, float(d.abs().max()))
+        del d
+    den = Xv.shape[1] * torch.view_as_real(W).pow(2).sum(dim=(1, 2))
+    return torch.sqrt(num / den).cpu().numpy(), dmax
+
+
+def test_cfg4_timed_plan_full_physics_every_element_50_steps(mmf, torch, orc):
+    p, ps, small, X = tiled_cfg4(torch)
+    pl = plan_for(mmf, p)
+    pl.propagate(X, p.steps)
+    torch.cuda.synchronize()
+    assert p.steps == 50 and tuple(X.shape) == (240, 1 << 22)
+    want = orc.rk4ip(small, ps.dt, ps.h, ps.alpha, ps.beta, ps.gamma, ps.kappa, p.steps)
+    lin = orc.rk4ip(small, ps.dt, ps.h, ps.alpha, ps.beta, 0.0, ps.kappa, p.steps)
+    assert workloads.rel_l2_per_field(want, lin).min() > 1e-2          # the nonlinearity matters over these 50 steps
+    err, dmax = tiled_error(torch, X, want)
+    assert err.max() <= TOL_FIELD, (err.max(), err.argmax(), dmax)
+    assert dmax <= 1e-9 * float(np.abs(want).max())                      # no single element is off either
+
+
+def test_cfg4_timed_plan_ssfm_every_element_50_steps(mmf, torch, orc):
+    p, ps, small, X = tiled_cfg4(torch, scale=2.0)
+    pl = plan_for(mmf, p)
+    pl.propagate_ssfm(X, p.steps)
+    torch.cuda.synchronize()
+    want = orc.ssfm_rk4(small, ps.dt, ps.h, ps.alpha, ps.beta, ps.gamma, ps.kappa, p.steps)
+    err, dmax = tiled_error(torch, X, want)
+    assert err.max() <= TOL_FIELD, (err.max(), err.argmax(), dmax)
+
+
+# -------------------------------------------------------- configs 2 and 3 at FULL size and FULL step count (golden)
+# The oracle needs ~30-45 min per config for these, so its output is stored, sampled, by tests/golden/make_golden.py
+# (a committed script that calls only oracle/ and workloads.py; its header has the command).
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_length_matches_golden(mmf, torch, cfg):
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg%d_full.npz" % cfg)
+    g = np.load(path)
+    p = workloads.problem(cfg)
+    assert list(g["meta"]) == [cfg, p.M, p.N, p.steps]
+    A = field_threaded(p)
+    pl = plan_for(mmf, p)
+    X = torch.from_numpy(A).to("cuda:0")
+    pl.propagate(X, p.steps)
+    torch.cuda.synchronize()
+    dev = X.device
+    rows, idx_d, idx_a = (torch.from_numpy(g[k]).to(dev) for k in ("rows_dense", "idx_dense", "idx_all"))
+    got_d = X[rows][:, idx_d].cpu().numpy()
+    got_a = X[:, idx_a].cpu().numpy()
+    norm2 = (X.real ** 2 + X.imag ** 2).sum(dim=1).cpu().numpy()
+    err_d = workloads.rel_l2_per_field(got_d, g["dense"])
+    err_a = workloads.rel_l2_per_field(got_a, g["all"])
+    assert err_d.max() <= TOL_FIELD, (err_d.max(), err_d.argmax())
+    assert err_a.max() <= TOL_FIELD, (err_a.max(), err_a.argmax())
+    assert np.abs(norm2 / g["norm2"] - 1.0).max() <= 1e-10

@@ -86,7 +86,9 @@ def test_forward_transform_integer_exact(mmf, torch, orc, logn):
 
 # ------------------------------------------------------------------------------------------------ linear operator D
 @pytest.mark.parametrize("cfg,M,logn", [(0, 2, 12), (1, 3, 13), (1, 2, 16), (2, 3, 14), (3, 5, 18), (4, 2, 15), (4, 1, 4),
-                                        (4, 1, 22), (4, 1, 23)])
+                                        (4, 1, 22), (4, 1, 23)] +
+                         # every transform length the plan accepts (each (N1, N2) split is its own instantiation)
+                         [(4, 1 + (logn & 1), logn) for logn in range(5, 25) if logn not in (12, 13, 14, 15, 16, 18, 22, 23)])
 def test_linear_operator_matches_oracle(mmf, torch, orc, cfg, M, logn):
     p = workloads.problem(cfg, M=M, N=1 << logn)
     A = p.field()
@@ -149,13 +151,15 @@ CASES = [
     (0, 2, 12, 100),      # config 0 at full size and step count
     (1, 6, 13, 40),
     (1, 6, 16, 12),       # config 1 at full size, shortened
-    (1, 6, 16, 250),      # config 1 at full size, a quarter of its 1000 steps: rounding errors stay far below the bar
+    (1, 6, 16, 1000),     # config 1 at full size and step count
     (2, 36, 14, 8),
     (3, 120, 13, 4),
     (4, 120, 14, 3),
     (4, 7, 18, 3),        # config-4 physics at the 2^18 transform size, odd mode count
     (3, 124, 13, 2),      # more than 120 modes: the DFMA nonlinear kernels and the four-buffer plan
     (4, 1, 23, 1),        # N = 2^23: N1 = 2^12, one-column tiles (W = 1) inside 16-column blocks
+    (4, 2, 17, 2), (4, 1, 19, 2), (4, 2, 20, 1), (4, 1, 21, 1), (4, 1, 24, 1),   # the remaining (N1, N2) splits
+    (0, 1, 5, 3), (0, 2, 8, 3), (0, 1, 9, 3), (0, 2, 10, 3),                      # short single-pass transforms
 ]
 
 

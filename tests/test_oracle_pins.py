@@ -301,3 +301,37 @@ def test_paper_printed_sizes():
             assert rows * N * b == want * (1 << 20)
         n += 1
     assert n == 6
+
+
+# ------------------------------------------------------- pins at the sizes / phases the oracle is the authority for
+def test_fft_equals_library_fft_at_full_length(orc):
+    """The oracle's radix-2 FFT is the authority at N = 2^22 (config 4): one row against numpy's pocketfft there."""
+    N = 1 << 22
+    x = rand_c(np.random.default_rng(22), N)
+    assert rel(orc.fft(x, -1), np.fft.fft(x)) <= 5e-15
+    assert rel(orc.fft(x, +1), N * np.fft.ifft(x)) <= 5e-15
+
+
+def test_tone_eigenvalue_at_large_phase_against_mpmath(orc):
+    """Config 4's dispersion phase (h/2) sum_n beta_n w^n / n! reaches ~4e3 rad at the band edge (hard
+    part 1).  A tone exp(-i W t) at such bins, gamma = 0: the output must be exp(h L(W)) times the input with the
+    eigenvalue computed by mpmath at 50 digits from Eq. (1)'s symbol — an fp64 evaluation of the phase would be off by
+    ~1e-12 here, a sign or 1/n! slip by O(1)."""
+    import mpmath as mp
+    mp.mp.dps = 50
+    N, dt, h, alpha = 1 << 14, 0.0625, 250.0, 4.6e-5
+    beta = np.array([[1.7e-4, 4.9e-2, -2.5e-2, 1.0e-4]])
+    worst_phase = 0.0
+    for j in (8190, -8191, 5000, -N // 2):
+        W = 2 * mp.pi * mp.mpf(j) / (mp.mpf(N) * mp.mpf(dt))
+        sym = sum(mp.mpf(float(b)) * W ** n / mp.factorial(n) for n, b in enumerate(beta[0]))
+        worst_phase = max(worst_phase, abs(float(sym * h / 2)))
+        lam = mp.exp((-mp.mpf(alpha) / 2 + 1j * sym) * mp.mpf(h))            # one step = two exp(h/2 L)
+        t = np.arange(N)
+        A = np.zeros((2, N), dtype=complex)
+        A[0] = np.exp(-2j * np.pi * ((j * t) % N) / N)                        # exp(-i W t), exact index reduction
+        A[1] = 0.5j * A[0]
+        out = orc.rk4ip(A, dt, h, alpha, beta, 0.0, np.eye(1), 1)
+        want = complex(lam) * A
+        assert rel(out, want) <= 2e-13, (j, rel(out, want))
+    assert worst_phase > 3e3                                                   # the regime the pin is for
