@@ -32,10 +32,19 @@ def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the committed `ncu --set full` capture of this
-# command on cfg4 (profiles/r1h_ncu_full_cfg4.md); other workloads have no capture: traffic = null.
-NCU_TRAFFIC_CFG4 = {"k_rows": 74.32e9, "k_cols<fwd>": 65.62e9, "k_cols<inv>": 65.47e9, "k_nlm<s23>": 64.38e9,
-                    "k_nlm<final_next>": 64.36e9}
+def load_counters(cfg):
+    """Per-kernel ncu counters (DRAM traffic, fp64 thread instructions per launch) of the newest committed
+    `ncu --set full` capture of this command: profiles/r*_counters_cfg<cfg>.json, written by
+    paper_1901_01895_b200/ncu_summary.py.  Returns (kernels, file, stale): stale = the kernel sources have changed since
+    the capture (then the numbers are NOT reported: traffic = null)."""
+    import glob
+    from paper_1901_01895_b200 import ncu_summary
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_counters_cfg%d.json" % cfg)))
+    if not files:
+        return {}, None, False
+    with open(files[-1]) as f:
+        d = json.load(f)
+    return d.get("kernels", {}), os.path.relpath(files[-1], ROOT), d.get("source_sha256") != ncu_summary.source_hash()
 
 
 def load_peaks():
@@ -130,25 +139,52 @@ def oracle_sample(cfg):
     return p, p.field()
 
 
-def oracle_steps(p, A, steps, nthreads):
+def oracle_steps(p, A, steps, nthreads, method="rk4ip"):
     from oracle import oracle as orc
+    fn = {"rk4ip": orc.rk4ip, "ssfm": orc.ssfm_rk4}[method]
     t0 = time.perf_counter()
-    orc.rk4ip(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, steps, nthreads=nthreads)
+    fn(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, steps, nthreads=nthreads)
     return time.perf_counter() - t0
 
 
-def time_oracle(cfg, budget_s):
-    """cpu_baseline leg: the oracle as it stands, all host cores, about `budget_s` seconds of work."""
+def host_description():
+    """CPU model string and available RAM of the box the oracle is timed on."""
+    model, avail = "unknown", None
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemAvailable"):
+                    avail = round(int(line.split()[1]) / 2 ** 20, 1)
+                    break
+    except OSError:
+        pass
+    return model, avail
+
+
+def time_oracle(cfg, budget_s, method="rk4ip"):
+    """cpu_baseline leg: the oracle as it stands (UNOPTIMISED: textbook radix-2 transform, -O2, stage sums on one
+    thread), all host cores, about `budget_s` seconds of work; plus the single-core figure on configs 0 and 1."""
     from oracle import oracle as orc
+    from paper_1901_01895_b200 import workloads
     orc.build()
     p, A = oracle_sample(cfg)
     nthreads = orc.default_threads()
-    t1 = oracle_steps(p, A, 1, nthreads)
+    t1 = oracle_steps(p, A, 1, nthreads, method)
     steps = int(max(1, min(500, budget_s / max(t1, 1e-3))))
-    dt = oracle_steps(p, A, steps, nthreads)
-    sample = "cfg%d recipe with N cut to 2^%d (M=%d, %d rows), %d steps in %.1f s" % (
-        cfg, p.N.bit_length() - 1, p.M, p.R, steps, dt)
-    return p.R * p.N * steps / dt, nthreads, sample
+    dt = oracle_steps(p, A, steps, nthreads, method)
+    sample = "cfg%d recipe with N cut to 2^%d (M=%d, %d rows), %d %s steps in %.1f s" % (
+        cfg, p.N.bit_length() - 1, p.M, p.R, steps, method, dt)
+    single = {}
+    for c, st in ((0, 20), (1, 2)):
+        q = workloads.problem(c)
+        ts = oracle_steps(q, q.field(), st, 1, method)
+        single["cfg%d" % c] = q.R * q.N * st / ts
+    return p.R * p.N * steps / dt, nthreads, sample, single
 
 
 def run_reference(args):
@@ -160,22 +196,95 @@ def run_reference(args):
     orc.build()
     p, A = oracle_sample(args.cfg)
     nthreads = orc.default_threads()
+    method = "ssfm" if args.method == "ssfm" else "rk4ip"
     for _ in range(args.warmup):
-        oracle_steps(p, A, 1, nthreads)
+        oracle_steps(p, A, 1, nthreads, method)
     tsum = 0.0
     for _ in range(args.steps):
-        tsum += oracle_steps(p, A, 1, nthreads)
+        tsum += oracle_steps(p, A, 1, nthreads, method)
     value = p.R * p.N * args.steps / tsum
-    sample = "each step = 1 RK4IP step of the cfg%d recipe with N cut to 2^%d (M=%d, %d rows)" % (
-        args.cfg, p.N.bit_length() - 1, p.M, p.R)
+    sample = "each step = 1 %s step of the cfg%d recipe with N cut to 2^%d (M=%d, %d rows)" % (
+        method, args.cfg, p.N.bit_length() - 1, p.M, p.R)
+    model, avail = host_description()
+    full = workloads.problem(args.cfg)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tsum / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_string(workloads.problem(args.cfg)), "l2": "n/a (CPU oracle)"},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": nthreads, "kind": "oracle", "sample": sample},
+            "config": {"workload": workload_string(full) + (
+                           " -- THIS ARM RAN A BOUNDED SAMPLE OF IT: N cut from 2^%d to 2^%d, everything else unchanged"
+                           % (full.N.bit_length() - 1, p.N.bit_length() - 1) if p.N != full.N else ""),
+                       "workload_run": workload_string(p), "method": method, "l2": "n/a (CPU oracle)"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": nthreads, "kind": "oracle",
+                             "note": "unoptimised test infrastructure (textbook radix-2, -O2)", "sample": sample, "cpu_model": model, "mem_available_GiB": avail},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ measurement probes
+def run_probes(args):
+    """--probes: the denominators DESIGN.md §6 quotes, measured live through the C ABI (mmf_probe_fp64,
+    mmf_probe_tma_copy): fp64 issue peaks of the plain and the tensor (DMMA) path, and what a pure TMA copy through
+    the product kernels' ring reaches with each kernel's access pattern on a config-4 sized buffer."""
+    import torch
+    from paper_1901_01895_b200 import binding
+    assert torch.cuda.is_available()
+    binding.lib()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    sampler = ClockSampler(0)
+    sampler.start()
+    fp = []
+    names = ["DADD x=x+y", "DMUL x=x*y", "DFMA x=fma(y,z,x) (3 distinct regs)", "DFMA x=fma(x,y,y) (2 distinct regs)",
+             "add/sub butterfly (2 DADD)", "DMMA m8n8k4 (4 chains per warp)"]
+    for kind, name in enumerate(names):
+        for threads in (512, 1024):
+            ms, n = binding.probe_fp64(kind, threads=threads, iters=4000)
+            e = {"kind": name, "threads_per_sm": threads, "ms": round(ms, 3)}
+            if kind == 5:
+                e["TFLOP_s"] = round(n * 512 / (ms * 1e-3) / 1e12, 2)
+                e["warp_inst_per_s_per_sm"] = n / (ms * 1e-3) / sms
+            else:
+                e["thread_inst_per_s_per_sm"] = n / (ms * 1e-3) / sms
+                e["TFLOP_s"] = round(n * (2 if kind in (2, 3) else 1) / (ms * 1e-3) / 1e12, 2)
+            fp.append(e)
+    clocks = sampler.stop()
+    clk = (clocks.get("sm_mhz") or 1965.0) * 1e6
+    for e in fp:
+        if "thread_inst_per_s_per_sm" in e:
+            e["thread_inst_per_clk_per_sm"] = round(e.pop("thread_inst_per_s_per_sm") / clk, 1)
+        else:
+            e["clk_per_dmma_per_sm"] = round(clk / e.pop("warp_inst_per_s_per_sm"), 2)
+    R, N, N1, N2 = 240, 1 << 22, 1 << 10, 1 << 12
+    buf = torch.zeros(R * N * 16, dtype=torch.uint8, device=dev)
+    # (name, dim0 [doubles], dim1 [rows], stride [B], box0, box1, nbox, nct_log, c0_mul, c1_mul, ntiles, slots, bulk)
+    cases = [
+        ("contiguous 64 KiB tiles (cp.async.bulk; pass B, natural order)", 0, 0, 0, 8192, 1, 1, 0, 0, 0, R * N // 4096, 3, 1),
+        ("64 B segments at 64 KiB pitch, 1024 rows per tile (passes A/C, natural order)",
+         2 * N2, R * N1, N2 * 16, 8, 256, 4, 10, 8, 1024, R * N2 // 4, 3, 0),
+        ("64 B segments at 256 B pitch inside a contiguous block (passes A/C, blocked order WB=16)",
+         32, R * (N2 // 16) * N1, 256, 8, 256, 4, 2, 8, 1024, R * N2 // 4, 3, 0),
+        ("64 B segments at 128 B pitch (passes A/C, WB=8)", 16, R * (N2 // 8) * N1, 128, 8, 256, 4, 1, 8, 1024, R * N2 // 4, 3, 0),
+        ("64 B segments at 1 KiB pitch (passes A/C, WB=64)", 128, R * (N2 // 64) * N1, 1024, 8, 256, 4, 4, 8, 1024, R * N2 // 4, 3, 0),
+        ("256 B segments at 256 KiB pitch (pass B, blocked order WB=16)",
+         2 * N1 * 16, R * (N2 // 16), N1 * 16 * 16, 32, 256, 1, 10, 32, 256, R * N1, 3, 0),
+        ("128 B segments at 128 KiB pitch (pass B, WB=8)", 2 * N1 * 8, R * (N2 // 8), N1 * 8 * 16, 16, 256, 2, 10, 16, 512, R * N1, 3, 0),
+        ("128 B segments at 64 MiB pitch, 240 rows per tile (nonlinear kernels, 8-sample tile)",
+         2 * N, R, N * 16, 16, R, 1, 30, 16, 0, N // 8, 3, 0),
+        ("same, 6 slots", 2 * N, R, N * 16, 16, R, 1, 30, 16, 0, N // 8, 6, 0),
+        ("256 B segments at 64 MiB pitch, 240 rows per tile (16-sample tile)", 2 * N, R, N * 16, 32, R, 1, 30, 32, 0, N // 16, 3, 0),
+    ]
+    tma = []
+    for c in cases:
+        name, d0, d1, st, b0, b1, nbox, ncl, c0m, c1m, nt, slots, bulk = c
+        ms, by = binding.probe_tma_copy(buf, d0, d1, st, b0, b1, nbox, ncl, c0m, c1m, nt, slots=slots, bulk=bulk, reps=3)
+        tma.append({"pattern": name, "tile_bytes": nbox * b0 * b1 * 8, "slots": slots, "ms": round(ms, 3),
+                    "GB_s": round(by / (ms * 1e-3) / 1e9, 0), "GB_moved": round(by / 1e9, 1)})
+    peak, src = load_peaks()
+    print(json.dumps({"probes": {"fp64": fp, "tma_copy": tma}, "sms": sms, "clocks_during_fp64": clocks,
+                      "hbm_peak_GB_s": peak, "hbm_peak_source": src}), flush=True)
     return 0
 
 
@@ -257,7 +366,7 @@ def run_mmf(args):
 
     # ---- roofline of the dominant kernel (largest summed device time in the timed region) ----
     peak, peak_src = load_peaks()
-    full_cfg4 = args.cfg == 4 and args.modes is None and args.logn is None and args.method == "rk4ip"
+    full_cfg = args.modes is None and args.logn is None and args.method == "rk4ip"
     roof = None
     breakdown = []
     tot_kernel_ms = sum(k["total_ms"] for k in kern) or 1.0
@@ -270,19 +379,23 @@ def run_mmf(args):
         top = max(kern, key=lambda k: k["total_ms"])
         avg = top["total_ms"] / top["launches"]
         ach = top["alg_bytes_per_launch"] / (avg * 1e-3) / 1e9
+        counters, cfile, stale = load_counters(args.cfg) if full_cfg else ({}, None, False)
+        ctr = {} if stale else counters.get(top["name"], {})
         roof = {"bound": "hbm", "kernel": top["name"], "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": NCU_TRAFFIC_CFG4.get(top["name"]) if full_cfg4 else None,
-                "traffic_source": "profiles/r1h_ncu_full_cfg4.md" if full_cfg4 else None, "peak_source": peak_src,
+                "frac": ach / peak, "traffic": ctr.get("traffic_bytes"),
+                "traffic_source": (cfile + (" (STALE: kernel sources changed since the capture; not reported)" if stale else ""))
+                if cfile else None, "peak_source": peak_src,
                 "alg_bytes_per_launch": top["alg_bytes_per_launch"], "avg_launch_ms": avg}
-        if full_cfg4 and top["name"] == "k_rows":
+        if ctr.get("fp64_thread_inst"):
             # second bound of the same kernel: fp64 issue.  Thread-level fp64 instructions of one launch from the
-            # committed ncu capture (smsp__inst_executed x fp64 share, profiles/r1h_ncu_full_cfg4.md); peak = 64 per
-            # clock per SM x 148 SMs (measured with a DADD / DMUL stream) at the clock seen under load.
-            fp64_inst = 1.69e11
+            # committed capture (dadd + dmul + dfma counters); peak = 64 per clock per SM x the SM count
+            # (profiles/r2_probes.md: measured with DADD / DMUL streams) at the clock seen under load.
             clk = (clocks.get("sm_mhz") or 1965.0) * 1e6
-            peak_i = 64.0 * 148 * clk
-            roof["fp64_issue"] = {"achieved_Tinst_s": fp64_inst / (avg * 1e-3) / 1e12, "peak_Tinst_s": peak_i / 1e12,
-                                  "frac": fp64_inst / (avg * 1e-3) / peak_i, "sm_mhz": clk / 1e6}
+            peak_i = 64.0 * torch.cuda.get_device_properties(dev).multi_processor_count * clk
+            roof["fp64_issue"] = {"thread_inst_per_launch": ctr["fp64_thread_inst"],
+                                  "achieved_Tinst_s": ctr["fp64_thread_inst"] / (avg * 1e-3) / 1e12,
+                                  "peak_Tinst_s": peak_i / 1e12, "frac": ctr["fp64_thread_inst"] / (avg * 1e-3) / peak_i,
+                                  "sm_mhz": clk / 1e6}
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
     if args.method == "rk4ip":
         balg = (36 if p.N > 4096 else 20) * F
@@ -325,8 +438,12 @@ def run_mmf(args):
     # ---- the CPU oracle, timed on this box's host cores on a bounded sample ----
     cpu = None
     if not args.no_cpu:
-        fss, cores, sample = time_oracle(args.cfg, budget_s=args.cpu_seconds)
-        cpu = {"value": fss, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        fss, cores, sample, single = time_oracle(args.cfg, budget_s=args.cpu_seconds,
+                                                 method="ssfm" if args.method == "ssfm" else "rk4ip")
+        model, avail = host_description()
+        cpu = {"value": fss, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+               "note": "the oracle is unoptimised test infrastructure (textbook radix-2, -O2): a baseline, not a target",
+               "single_core": single, "cpu_model": model, "mem_available_GiB": avail}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -360,7 +477,11 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT reference point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--probes", action="store_true",
+                    help="measure the fp64 issue peaks and the TMA access-pattern ceilings instead of the benchmark")
     args = ap.parse_args()
+    if args.probes:
+        return run_probes(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_mmf(args)
