@@ -141,7 +141,7 @@ def oracle_sample(cfg):
 
 def oracle_steps(p, A, steps, nthreads, method="rk4ip"):
     from oracle import oracle as orc
-    fn = {"rk4ip": orc.rk4ip, "ssfm": orc.ssfm_rk4}[method]
+    fn = {"rk4ip": orc.rk4ip, "ssfm": orc.ssfm_rk4, "agrawal": orc.ssfm_agrawal}[method]
     t0 = time.perf_counter()
     fn(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, steps, nthreads=nthreads)
     return time.perf_counter() - t0
@@ -196,7 +196,7 @@ def run_reference(args):
     orc.build()
     p, A = oracle_sample(args.cfg)
     nthreads = orc.default_threads()
-    method = "ssfm" if args.method == "ssfm" else "rk4ip"
+    method = args.method
     for _ in range(args.warmup):
         oracle_steps(p, A, 1, nthreads, method)
     tsum = 0.0
@@ -326,7 +326,8 @@ def run_mmf(args):
         torch.cuda.synchronize()
 
     # ---- warm-up (W untimed steps), then K timed steps, field resident in HBM ----
-    advance = plan.propagate if args.method == "rk4ip" else plan.propagate_ssfm
+    advance = {"rk4ip": plan.propagate, "ssfm": plan.propagate_ssfm,
+               "agrawal": lambda X_, n_: plan.propagate_ssfm_agrawal(X_, n_, niter=args.niter)}[args.method]
     advance(X, args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
@@ -399,6 +400,8 @@ def run_mmf(args):
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
     if args.method == "rk4ip":
         balg = (36 if p.N > 4096 else 20) * F
+    elif args.method == "agrawal":                  # (1 + niter) D on one buffer + S0 (1.25 F), IT1 (2.25 F), ITJ (3.25 F)
+        balg = ((1 + args.niter) * (6 if p.N > 4096 else 2) + 3.5 + 3.25 * (args.niter - 1)) * F
     else:                                           # two D on one buffer (3 passes x 2 F, or 2 F on chip) + 2 F
         balg = (14 if p.N > 4096 else 6) * F
     t_roof_ms = balg / (peak * 1e9) * 1e3
@@ -439,7 +442,7 @@ def run_mmf(args):
     cpu = None
     if not args.no_cpu:
         fss, cores, sample, single = time_oracle(args.cfg, budget_s=args.cpu_seconds,
-                                                 method="ssfm" if args.method == "ssfm" else "rk4ip")
+                                                 method=args.method)
         model, avail = host_description()
         cpu = {"value": fss, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                "note": "the oracle is unoptimised test infrastructure (textbook radix-2, -O2): a baseline, not a target",
@@ -470,8 +473,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json config id (default 4: M=120, N=2^22)")
     ap.add_argument("--impl", default="mmf", choices=["mmf", "reference"])
-    ap.add_argument("--method", default="rk4ip", choices=["rk4ip", "ssfm"],
-                    help="rk4ip (Eq. 6, the headline path) or ssfm (SSFM-RK4, the symmetric split step of Eq. 4)")
+    ap.add_argument("--method", default="rk4ip", choices=["rk4ip", "ssfm", "agrawal"],
+                    help="rk4ip (Eq. 6, the headline path), ssfm (SSFM-RK4) or agrawal (SSFM-Agrawal): the symmetric "
+                         "split step of Eq. 4 with a Runge-Kutta resp. an iterative nonlinear part")
+    ap.add_argument("--niter", type=int, default=2, help="iterations per step of --method agrawal")
     ap.add_argument("--modes", type=int, default=None, help="override the config's mode count M (extra data points)")
     ap.add_argument("--logn", type=int, default=None, help="override the config's N = 2^logn (extra data points)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

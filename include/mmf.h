@@ -46,7 +46,8 @@ int mmf_plan_create(mmf_plan **out, int M, long long N, double dt, double h, dou
                     double gamma, const double *kappa);
 
 /* Bytes of device workspace the plan needs: one more full-field buffer when N <= 4096, two when N > 4096 (three resp.
- * four when M > 120) plus the tabulated exp(h/2 L_a(w_k)) of Eq. (6a) (one row per mode).  The caller allocates it
+ * four when M > 120) plus the tabulated exp(h/2 L_a(w_k)) of Eq. (6a) (one row per mode), plus for N <= 4096 a real
+ * [M][N] table for mmf_propagate_ssfm_agrawal.  The caller allocates it
  * (e.g. a torch uint8 tensor), 256-byte aligned, and keeps it alive while the plan is used.  Note: for N > 4096 the
  * library works on copies in an internal (blocked) sample order; A_dev is read in the natural order documented above
  * by the first kernel of a call and written in it by the last one. */
@@ -67,6 +68,15 @@ int mmf_propagate(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
  * Same arguments and layout as mmf_propagate; runs on the same transform kernels and one fused nonlinear kernel that
  * evaluates all four N per sample tile (2 F of traffic).  Requires M <= 120 (MMF_EINVAL otherwise). */
 int mmf_propagate_ssfm(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
+
+/* Advance A by nsteps symmetric split steps with the ITERATIVE nonlinear part ("SSFM-Agrawal": Eq. 4 PAPER.md:58-61,
+ * "solved by an iterative approach as described in [6]" PAPER.md:63, "|A|^2 once at the position z for the first
+ * iteration and at the position z + h for every following iteration" PAPER.md:111), in place.  Per step, with
+ * S_a(u) = sum_b kappa_ab |u_b|^2 and the integral of Eq. (4) by the trapezoidal rule:
+ *   B = exp(h/2 L) A(z);  A_1 = exp(h/2 L)[exp(i h gamma S(A(z))) B];
+ *   A_j = exp(h/2 L)[exp(i (h gamma/2) (S(A(z)) + S(A_{j-1}))) B], j = 2..niter;  A(z+h) = A_niter.   (globally O(h^2))
+ * niter >= 1 (2 is the textbook choice).  Same arguments, layout and M <= 120 restriction as mmf_propagate_ssfm. */
+int mmf_propagate_ssfm_agrawal(mmf_plan *plan, void *A_dev, int nsteps, int niter, void *cuda_stream);
 
 /* Same, for a HOST field: copies A_host to an internal slot of the workspace-adjacent device buffer `A_dev_scratch`
  * (device, [2M][N] complex128, caller-owned), propagates, copies back and SYNCHRONISES the stream.  A_host should be

@@ -41,8 +41,9 @@ def lib():
         L.orc_nonlinear.argtypes = [dp, dp, i, ll, d, dp, i]
         L.orc_rk4ip.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
         L.orc_ssfm_rk4.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
+        L.orc_ssfm_agrawal.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i, i]
         for f in (L.orc_dft, L.orc_fft, L.orc_omega, L.orc_linear_table, L.orc_apply_D, L.orc_nonlinear,
-                  L.orc_rk4ip, L.orc_ssfm_rk4):
+                  L.orc_rk4ip, L.orc_ssfm_rk4, L.orc_ssfm_agrawal):
             f.restype = i
         _lib = L
     return _lib
@@ -136,4 +137,21 @@ def ssfm_rk4(A, dt, h, alpha, beta, gamma, kappa, nsteps, nthreads=None):
         nthreads = default_threads()
     rc = lib().orc_ssfm_rk4(_p(A), M, N, dt, h, alpha, _p(beta), beta.shape[1], gamma, _p(kappa), nsteps, nthreads)
     assert rc == 0, "orc_ssfm_rk4 rejected its arguments"
+    return A
+
+
+def ssfm_agrawal(A, dt, h, alpha, beta, gamma, kappa, nsteps, niter=2, nthreads=None):
+    """Return A advanced nsteps SSFM-Agrawal steps (symmetric split step, iterative trapezoidal nonlinear part with
+    niter iterations per step; Eq. 4, reading R14).  Same arguments as rk4ip."""
+    A = _c128(A).copy()
+    R, N = A.shape
+    M = R // 2
+    assert R == 2 * M
+    beta = _f64(beta).reshape(M, -1)
+    kappa = _f64(kappa).reshape(M, M)
+    if nthreads is None:
+        nthreads = default_threads()
+    rc = lib().orc_ssfm_agrawal(_p(A), M, N, dt, h, alpha, _p(beta), beta.shape[1], gamma, _p(kappa), nsteps, niter,
+                                nthreads)
+    assert rc == 0, "orc_ssfm_agrawal rejected its arguments"
     return A

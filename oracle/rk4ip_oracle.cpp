@@ -248,6 +248,56 @@ void ssfm_rk4_step(cplx* A, int M, long long N, const cplx* E, double hgamma, co
   apply_D(A, M, N, E, nthreads);
 }
 
+// S_a[t] = sum_b kappa_ab P_b[t],  P_b = |u_bx|^2 + |u_by|^2  (the real factor of N = i gamma S, Eq. 1)
+// for every mode a and sample t; S is [M][N] doubles.  Same plain loops and summation order as nonlinear().
+void mode_phase_rate(const cplx* u, double* S, int M, long long N, const double* kappa, int nthreads) {
+  const long long BLK = 4096;
+  long long nblk = (N + BLK - 1) / BLK;
+  parallel_for(nblk, nthreads, [&](long long blk) {
+    std::vector<double> P(M);
+    long long t0 = blk * BLK, t1 = std::min(N, t0 + BLK);
+    for (long long t = t0; t < t1; ++t) {
+      for (int b = 0; b < M; ++b) {
+        cplx ux = u[(2LL * b) * N + t], uy = u[(2LL * b + 1) * N + t];
+        P[b] = (ux.real() * ux.real() + ux.imag() * ux.imag()) + (uy.real() * uy.real() + uy.imag() * uy.imag());
+      }
+      for (int a = 0; a < M; ++a) {
+        double acc = 0.0;
+        for (int b = 0; b < M; ++b) acc += kappa[(long long)a * M + b] * P[b];
+        S[(long long)a * N + t] = acc;
+      }
+    }
+  });
+}
+
+// One symmetric split step with the ITERATIVE nonlinear part ("SSFM-Agrawal": Eq. 4, "solved by an
+// iterative approach as described in [6]" PAPER.md:63; "requires the computation of |A|^2 once at the position z for
+// the first iteration and at the position z + h for every following iteration" PAPER.md:111).  Reading R14:
+// the integral of Eq. (4) by the trapezoidal rule, int_z^{z+h} N(z') dz' ~ (h/2) [N(z) + N(z+h)] with N = i gamma S
+// (a multiplication in the time domain); N(z+h) is not known, so
+//   iteration 1:      N(z+h) := N(z)                        A_1 = D( exp(i h gamma S(A(z)))                  D A(z) )
+//   iteration j >= 2: N(z+h) from A_{j-1}                   A_j = D( exp(i (h gamma / 2) [S(A(z)) + S(A_{j-1})]) D A(z) )
+// and A(z+h) = A_niter.  D = exp(h/2 L), E its table (hh = h/2).  S0, S1 are [M][N] doubles, B and Y full fields.
+void ssfm_agrawal_step(cplx* A, int M, long long N, const cplx* E, double hgamma, const double* kappa, int niter,
+                       int nthreads, cplx* B, cplx* Y, double* S0, double* S1) {
+  const long long tot = 2LL * M * N;
+  mode_phase_rate(A, S0, M, N, kappa, nthreads);            // |A|^2 "once at the position z"
+  std::memcpy((void*)B, (const void*)A, sizeof(cplx) * tot);
+  apply_D(B, M, N, E, nthreads);                            // exp(h/2 L) A(z)
+  for (int it = 1; it <= niter; ++it) {
+    if (it > 1) mode_phase_rate(Y, S1, M, N, kappa, nthreads);   // |A|^2 "at the position z + h"
+    for (long long r = 0; r < 2LL * M; ++r) {
+      const double *s0 = S0 + (r / 2) * N, *s1 = S1 + (r / 2) * N;
+      for (long long t = 0; t < N; ++t) {
+        const double theta = (it == 1) ? hgamma * s0[t] : 0.5 * hgamma * (s0[t] + s1[t]);
+        Y[r * N + t] = B[r * N + t] * cplx(std::cos(theta), std::sin(theta));
+      }
+    }
+    apply_D(Y, M, N, E, nthreads);                          // exp(h/2 L)
+  }
+  std::memcpy((void*)A, (const void*)Y, sizeof(cplx) * tot);
+}
+
 }  // namespace
 
 extern "C" {
@@ -320,6 +370,21 @@ int orc_ssfm_rk4(double* A, int M, long long N, double dt, double h, double alph
   for (int s = 0; s < nsteps; ++s)
     ssfm_rk4_step((cplx*)A, M, N, E.data(), h * gamma, kappa, nthreads, k1.data(), k2.data(), k3.data(), k4.data(),
                   tmp.data());
+  return 0;
+}
+
+// A[2M][N] advanced nsteps SSFM-Agrawal steps of size h with niter >= 1 iterations each (Eq. 4, reading R14), in place.
+int orc_ssfm_agrawal(double* A, int M, long long N, double dt, double h, double alpha, const double* beta, int K,
+                     double gamma, const double* kappa, int nsteps, int niter, int nthreads) {
+  if (!A || !beta || !kappa || M < 1 || K < 1 || !is_pow2(N) || !(dt > 0) || nsteps < 0 || niter < 1) return -1;
+  if (nsteps == 0) return 0;
+  const long long tot = 2LL * M * N;
+  std::vector<cplx> E((size_t)M * N), B(tot), Y(tot);
+  std::vector<double> S0((size_t)M * N), S1((size_t)M * N);
+  linear_table(E.data(), M, N, dt, h / 2.0, alpha, beta, K, nthreads);
+  for (int s = 0; s < nsteps; ++s)
+    ssfm_agrawal_step((cplx*)A, M, N, E.data(), h * gamma, kappa, niter, nthreads, B.data(), Y.data(), S0.data(),
+                      S1.data());
   return 0;
 }
 

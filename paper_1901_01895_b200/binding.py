@@ -15,6 +15,7 @@ MMF_OK, MMF_EINVAL, MMF_ENOMEM, MMF_ECUDA = 0, -1, -2, -3
 
 # every symbol include/mmf.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["mmf_plan_create", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate", "mmf_propagate_ssfm",
+           "mmf_propagate_ssfm_agrawal",
            "mmf_propagate_host", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
            "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_set_timing", "mmf_kernel_class_count",
            "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version",
@@ -48,6 +49,8 @@ def lib():
     L.mmf_propagate.restype = i
     L.mmf_propagate_ssfm.argtypes = [vp, vp, i, vp]
     L.mmf_propagate_ssfm.restype = i
+    L.mmf_propagate_ssfm_agrawal.argtypes = [vp, vp, i, i, vp]
+    L.mmf_propagate_ssfm_agrawal.restype = i
     L.mmf_propagate_host.argtypes = [vp, vp, vp, i, vp]
     L.mmf_propagate_host.restype = i
     L.mmf_apply_linear.argtypes = [vp, vp, vp]
@@ -134,6 +137,11 @@ class Plan:
         """In-place SSFM-RK4 propagation (symmetric split step, Eq. 4) of a CUDA complex128 tensor [2M, N]."""
         _check(lib().mmf_propagate_ssfm(self._h, self._field_ptr(A), int(nsteps), _stream_ptr(stream)),
                "mmf_propagate_ssfm")
+
+    def propagate_ssfm_agrawal(self, A, nsteps, niter=2, stream=None):
+        """In-place SSFM-Agrawal propagation (symmetric split step, iterative trapezoidal nonlinear part)."""
+        _check(lib().mmf_propagate_ssfm_agrawal(self._h, self._field_ptr(A), int(nsteps), int(niter),
+                                                _stream_ptr(stream)), "mmf_propagate_ssfm_agrawal")
 
     def propagate_host(self, A_host, A_scratch, nsteps, stream=None):
         """A_host: pinned torch complex128 CPU tensor (2M, N); A_scratch: CUDA tensor of the same shape."""

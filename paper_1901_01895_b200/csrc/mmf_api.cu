@@ -121,6 +121,7 @@ struct mmf_plan {
   unsigned char* ws = nullptr;
   size_t ws_bytes = 0, field_bytes = 0;
   cpx *Y = nullptr, *Z = nullptr, *W = nullptr, *V = nullptr, *E = nullptr;
+  double* T = nullptr;  // N <= 4096: the table of mmf_propagate_ssfm_agrawal (workspace)
   long long launches = 0;
   // optional per-launch CUDA-event timing (mmf_plan_set_timing): one (start, stop) pair per launch
   bool timing = false;
@@ -133,11 +134,12 @@ namespace {
 
 // ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
 enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
-       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_NLM_ENTER, KC_NLM_EXIT, KC_PERM, KC_COUNT };
+       KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_NLM_ENTER, KC_NLM_EXIT, KC_NLM_AGR_S0,
+       KC_NLM_AGR_IT1, KC_NLM_AGR_ITJ, KC_PERM, KC_COUNT };
 const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
                                         "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>", "k_nlm<plain>",
                                         "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>", "k_nlm<enter>",
-                                        "k_nlm<exit>", "k_perm"};
+                                        "k_nlm<exit>", "k_nlm<agr_s0>", "k_nlm<agr_it1>", "k_nlm<agr_itj>", "k_perm"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
 struct LaunchTimer {
@@ -145,14 +147,14 @@ struct LaunchTimer {
   cudaStream_t st;
   cudaEvent_t stop = nullptr;
   // nfields = full-field copies the launch reads plus writes (its algorithmic traffic in units of F)
-  LaunchTimer(mmf_plan* p_, int kclass, int nfields, cudaStream_t st_) : p(p_), st(st_) {
+  LaunchTimer(mmf_plan* p_, int kclass, double nfields, cudaStream_t st_) : p(p_), st(st_) {
     if (!p->timing) return;
     cudaEvent_t a = nullptr;
     if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&stop) != cudaSuccess) { stop = nullptr; return; }
     p->ev.push_back(a);
     p->ev.push_back(stop);
     p->ev_class.push_back(kclass);
-    p->ev_bytes.push_back((double)nfields * (double)p->field_bytes);
+    p->ev_bytes.push_back(nfields * (double)p->field_bytes);
     cudaEventRecord(a, st);
   }
   ~LaunchTimer() {
@@ -390,8 +392,29 @@ int field_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
   return MMF_OK;
 }
 
+// tensor map of the real table T [M][N] doubles (the SSFM-Agrawal modes), box = 8 samples x M rows
+int table_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) {
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled is unavailable");
+    return MMF_ECUDA;
+  }
+  const cuuint64_t gdim[2] = {(cuuint64_t)p->N, (cuuint64_t)p->M};
+  const cuuint64_t gstride[1] = {(cuuint64_t)p->N * sizeof(double)};
+  const cuuint32_t box[2] = {MMF_NLM_T, (cuuint32_t)p->M};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return MMF_ECUDA;
+  }
+  return MMF_OK;
+}
+
 // PLAIN: A = U, B = OUT; ENTER: A = the caller's field (natural order), B = X, C = Y; EXIT: A = X, B = Y, C = the
-// caller's field; other modes: A = X, B = Y (C unused).
+// caller's field; AGR_*: A = X, B = Y, C = the real table T; other modes: A = X, B = Y (C unused).
 template <int NK, int MODE>
 int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st) {
   auto kern = k_nlt<NK, MODE>;
@@ -407,8 +430,11 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st) {
   int rc;
   if ((rc = field_tile_map(p, A, &mapA)) != MMF_OK) return rc;
   if ((rc = field_tile_map(p, B, &mapB)) != MMF_OK) return rc;
-  if ((rc = field_tile_map(p, C ? C : B, &mapC)) != MMF_OK) return rc;
-  const size_t smem = nlt_smem_bytes(p->M, NK, NARR);
+  if constexpr (nlm_has_table<MODE>()) {
+    if (!C) return MMF_EINVAL;
+    if ((rc = table_tile_map(p, C, &mapC)) != MMF_OK) return rc;
+  } else if ((rc = field_tile_map(p, C ? C : B, &mapC)) != MMF_OK) return rc;
+  const size_t smem = nlt_smem_bytes(p->M, NK, NARR, nlm_has_table<MODE>());
   const int threads = 32 * (q.NW + 1);
   CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
   int occ = 1;
@@ -416,7 +442,9 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st) {
   if (occ < 1) return MMF_EINVAL;
   long long grid = (long long)p->num_sms * occ;        // persistent: every resident CTA walks its own tile list
   if (grid > q.ntiles) grid = q.ntiles;
-  LaunchTimer lt(p, KC_NLM_PLAIN + MODE, (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 2 : (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT) ? 4 : 3, st);
+  constexpr double kFields = (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 2 : (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT) ? 4
+                             : MODE == NLM_AGR_S0 ? 1.25 : MODE == NLM_AGR_IT1 ? 2.25 : MODE == NLM_AGR_ITJ ? 3.25 : 3;
+  LaunchTimer lt(p, KC_NLM_PLAIN + MODE, kFields, st);
   kern<<<(unsigned)grid, threads, smem, st>>>(mapA, mapB, mapC, q);
   p->launches++;
   CU(cudaGetLastError());
@@ -568,7 +596,10 @@ size_t mmf_plan_workspace_bytes(const mmf_plan* p) {
   const size_t E = align_up(sizeof(cpx) * (size_t)p->M * (size_t)p->N, 256);
   // tensor-path plan: one more field buffer; DFMA plan (M > 120): three, plus one to hold the field in tiled order
   // (N > 4096, tensor path: two, the field and the second buffer both live in the workspace in blocked order)
-  return (p->nlm_nk > 0 ? (p->logn1 > 0 ? 2 : 1) : (p->logn1 > 0 ? 4 : 3)) * F + E;
+  // N <= 4096 (field sizes of KiB..MiB): also the real table T [M][N] of mmf_propagate_ssfm_agrawal; for N > 4096 T
+  // lives in the caller's field buffer, which is free between the entry and the exit conversion
+  const size_t T = p->logn1 > 0 ? 0 : align_up(sizeof(double) * (size_t)p->M * (size_t)p->N, 256);
+  return (p->nlm_nk > 0 ? (p->logn1 > 0 ? 2 : 1) : (p->logn1 > 0 ? 4 : 3)) * F + E + T;
 }
 
 int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_stream) {
@@ -589,6 +620,7 @@ int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_s
     p->V = p->logn1 > 0 ? (cpx*)(p->ws + 3 * F) : nullptr;
     p->E = (cpx*)(p->ws + (p->logn1 > 0 ? 4 : 3) * F);
   }
+  p->T = p->logn1 > 0 ? nullptr : (double*)((unsigned char*)p->E + align_up(sizeof(cpx) * (size_t)p->M * (size_t)p->N, 256));
   EtabParams P;
   memset(&P, 0, sizeof(P));
   static const dd TWO_PI_DD = {6.283185307179586232e+00, 2.449293598294706414e-16};
@@ -671,6 +703,35 @@ int mmf_propagate_ssfm(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) 
     if ((rc = apply_D(p, X, X, 1, st)) != MMF_OK) return rc;              // exp(h/2 L)
   }
   if (tiled && (rc = to_natural(p, X, A, st)) != MMF_OK) return rc;
+  return MMF_OK;
+}
+
+int mmf_propagate_ssfm_agrawal(mmf_plan* p, void* A_dev, int nsteps, int niter, void* cuda_stream) {
+  if (!p || !A_dev || nsteps < 0 || niter < 1 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
+  if (!p->ws || p->nlm_nk <= 0 || !on_plan_device(p)) return MMF_EINVAL;  // tensor-path nonlinear kernel only (M <= 120)
+  if (nsteps == 0) return MMF_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cpx* A = (cpx*)A_dev;
+  const bool tiled = p->logn1 > 0;
+  // two field buffers that swap roles every step (X: the field at z, then exp(h/2 L) A(z); Y: the iterate) and the
+  // real table T = h gamma S(A(z)).  N > 4096: both buffers in the workspace (blocked order), T in the caller's buffer.
+  cpx *X = tiled ? p->Y : A, *Y = tiled ? p->Z : p->Y;
+  double* T = tiled ? (double*)A : p->T;
+  int rc;
+  if (tiled && (rc = to_tiled(p, A, X, st)) != MMF_OK) return rc;
+  for (int s = 0; s < nsteps; ++s) {
+    if ((rc = launch_nlm<NLM_AGR_S0>(p, X, X, st, (cpx*)T)) != MMF_OK) return rc;      // |A|^2 "once at the position z"
+    if ((rc = apply_D(p, X, X, 1, st)) != MMF_OK) return rc;                            // exp(h/2 L) A(z)
+    if ((rc = launch_nlm<NLM_AGR_IT1>(p, X, Y, st, (cpx*)T)) != MMF_OK) return rc;     // iteration 1: N(z+h) := N(z)
+    if ((rc = apply_D(p, Y, Y, 1, st)) != MMF_OK) return rc;                            // exp(h/2 L)
+    for (int it = 2; it <= niter; ++it) {
+      if ((rc = launch_nlm<NLM_AGR_ITJ>(p, X, Y, st, (cpx*)T)) != MMF_OK) return rc;   // |A|^2 at z + h from the iterate
+      if ((rc = apply_D(p, Y, Y, 1, st)) != MMF_OK) return rc;
+    }
+    cpx* t = X; X = Y; Y = t;
+  }
+  if (tiled) return to_natural(p, X, A, st);
+  if (X != A) CU(cudaMemcpyAsync(A, X, p->field_bytes, cudaMemcpyDeviceToDevice, st));
   return MMF_OK;
 }
 

@@ -18,6 +18,11 @@
 //   NLM_RK4     X <- X + k1/6 + k2/3 + k3/3 + k4/6,  k1 = NL(X), k2 = NL(X + k1/2), k3 = NL(X + k2/2), k4 = NL(X + k3):
 //               the nonlinear substep of the symmetric split step (Eq. 4, "SSFM-RK4"): classical RK4
 //               over h of dA/dz = N(A) A, four contraction rounds per tile, the field read and written once (2 F).
+//   NLM_AGR_S0 / NLM_AGR_IT1 / NLM_AGR_ITJ   the nonlinear part of the ITERATIVE symmetric split step ("SSFM-Agrawal",
+//               Eq. 4; reading R14: trapezoidal rule with N(z+h) from the previous iterate):
+//               S0:  T <- hg S(X)                      (|A|^2 "once at the position z"; T is a real [M][N] table)
+//               IT1: Y <- exp(i T) X                   (first iteration, N(z+h) := N(z); X = exp(h/2 L) A(z))
+//               ITJ: Y <- exp(i (T + hg S(Y)) / 2) X   (later iterations, |A|^2 "at the position z + h" from Y)
 //
 // Design.  The kappa contraction S = kappa * P is a (M x M) x (M x 8) fp64 matrix product per tile: it runs on the
 // fp64 tensor path (mma.sync.m8n8k4.f64, SASS DMMA; tcgen05 has no fp64 kind).  Compute warp w owns mode rows
@@ -36,7 +41,8 @@
 
 namespace mmf {
 
-enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3, NLM_RK4 = 4, NLM_ENTER = 5, NLM_EXIT = 6 };
+enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3, NLM_RK4 = 4, NLM_ENTER = 5, NLM_EXIT = 6,
+       NLM_AGR_S0 = 7, NLM_AGR_IT1 = 8, NLM_AGR_ITJ = 9 };
 
 #define MMF_NLM_T 8           // time samples per tile
 #define MMF_NLM_PSTRIDE 12    // doubles per P row in shared memory (8 + 4: conflict-free B-fragment reads)
@@ -59,12 +65,21 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 }
 
 template <int MODE>
-__host__ __device__ constexpr int nlm_narr() { return (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 1 : 2; }  // arrays per slot
+__host__ __device__ constexpr int nlm_narr() {  // field arrays per slot
+  return (MODE == NLM_PLAIN || MODE == NLM_RK4 || MODE == NLM_AGR_S0 || MODE == NLM_AGR_IT1) ? 1 : 2;
+}
+template <int MODE>
+__host__ __device__ constexpr bool nlm_has_table() {  // the slot also holds a tile of the real table T (M x 8 doubles)
+  return MODE == NLM_AGR_S0 || MODE == NLM_AGR_IT1 || MODE == NLM_AGR_ITJ;
+}
 
 // bytes of dynamic shared memory: ring slots, two P buffers, mbarriers
-__host__ __device__ inline size_t nlt_slot_bytes(int M, int narr) { return (size_t)narr * 2 * M * MMF_NLM_T * sizeof(cpx); }
-__host__ __device__ inline size_t nlt_smem_bytes(int M, int nk, int narr) {
-  return MMF_NLM_SLOTS * nlt_slot_bytes(M, narr) + (size_t)2 * (4 * nk) * MMF_NLM_PSTRIDE * sizeof(double) + 128;
+__host__ __device__ inline size_t nlt_table_bytes(int M) { return ((size_t)M * MMF_NLM_T * sizeof(double) + 127) & ~(size_t)127; }
+__host__ __device__ inline size_t nlt_slot_bytes(int M, int narr, bool table) {
+  return (size_t)narr * 2 * M * MMF_NLM_T * sizeof(cpx) + (table ? nlt_table_bytes(M) : 0);
+}
+__host__ __device__ inline size_t nlt_smem_bytes(int M, int nk, int narr, bool table) {
+  return MMF_NLM_SLOTS * nlt_slot_bytes(M, narr, table) + (size_t)2 * (4 * nk) * MMF_NLM_PSTRIDE * sizeof(double) + 128;
 }
 
 // S = kappa_slab * P  for this warp's 8 rows and the tile's 8 samples (four independent accumulator chains)
@@ -85,7 +100,8 @@ __device__ __forceinline__ cpx axpy(double s, cpx a, cpx b) { return make_double
 
 // NK = ceil(M / 4) k-steps of the contraction (compile-time: the kappa fragments are a register array).
 // mapA / mapB: 2-D tensor maps (inner = 2N doubles, outer = 2M rows, box = 16 doubles x 2M rows) of
-//   PLAIN: U / OUT;  other modes: X / Y.
+//   PLAIN: U / OUT;  other modes: X / Y.  mapC: ENTER / EXIT the caller's field; AGR_*: the table T (inner = N doubles,
+//   outer = M rows, box = 8 doubles x M rows).
 // block = 32 (NW + 1) threads; grid = persistent; dynamic smem = nlt_smem_bytes(M, NK, narr).
 template <int NK, int MODE>
 __global__ void __launch_bounds__(512, 1)
@@ -97,7 +113,9 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int M = p.M, R = 2 * M, NW = p.NW;
   const size_t arr_elems = (size_t)R * MMF_NLM_T;            // cpx per array per slot
-  const size_t slot_bytes = NARR * arr_elems * sizeof(cpx);
+  constexpr bool TABLE = nlm_has_table<MODE>();
+  const size_t tab_off = NARR * arr_elems * sizeof(cpx);      // the table tile sits behind the field arrays of a slot
+  const size_t slot_bytes = tab_off + (TABLE ? nlt_table_bytes(M) : 0);
   double* Pb0 = reinterpret_cast<double*>(smem_raw + MMF_NLM_SLOTS * slot_bytes);
   double* Pb1 = Pb0 + 4 * NK * MMF_NLM_PSTRIDE;
   uint64_t* full = reinterpret_cast<uint64_t*>(Pb1 + 4 * NK * MMF_NLM_PSTRIDE);
@@ -137,6 +155,12 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
         tma_store_2d(&mapC, c0, 0, s + arr_elems * sizeof(cpx));
       } else if constexpr (MODE == NLM_EXIT) {  // the new field, natural order
         tma_store_2d(&mapC, (int)(natural_tile(tl) * 2 * MMF_NLM_T), 0, s);
+      } else if constexpr (MODE == NLM_AGR_S0) {  // only the table leaves
+        tma_store_2d(&mapC, (int)(tl * MMF_NLM_T), 0, s + tab_off);
+      } else if constexpr (MODE == NLM_AGR_IT1) {
+        tma_store_2d(&mapB, c0, 0, s);
+      } else if constexpr (MODE == NLM_AGR_ITJ) {
+        tma_store_2d(&mapB, c0, 0, s + arr_elems * sizeof(cpx));
       } else {
         tma_store_2d((MODE == NLM_PLAIN) ? &mapB : &mapA, c0, 0, s);
         if constexpr (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT) tma_store_2d(&mapB, c0, 0, s + arr_elems * sizeof(cpx));
@@ -154,10 +178,13 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
         store_tile(tile - MMF_NLM_SLOTS * tstep, slot);
         tma_store_wait_read();
       }
-      mbar_arrive_expect_tx(&full[slot], (uint32_t)(kLoadArrays * arr_elems * sizeof(cpx)));
+      constexpr bool kLoadTable = MODE == NLM_AGR_IT1 || MODE == NLM_AGR_ITJ;
+      mbar_arrive_expect_tx(&full[slot], (uint32_t)(kLoadArrays * arr_elems * sizeof(cpx) +
+                                                    (kLoadTable ? (size_t)M * MMF_NLM_T * sizeof(double) : 0)));
       const long long tin = (MODE == NLM_ENTER) ? natural_tile(tile) : tile;
       tma_load_2d(s, &mapA, (int)(tin * 2 * MMF_NLM_T), 0, &full[slot]);
       if constexpr (kLoadArrays == 2) tma_load_2d(s + arr_elems * sizeof(cpx), &mapB, (int)(tile * 2 * MMF_NLM_T), 0, &full[slot]);
+      if constexpr (kLoadTable) tma_load_2d(s + tab_off, &mapC, (int)(tile * MMF_NLM_T), 0, &full[slot]);
     }
     for (int jj = (j > MMF_NLM_SLOTS ? j - MMF_NLM_SLOTS : 0); jj < j; ++jj) {  // drain
       const int slot = jj % MMF_NLM_SLOTS, use = jj / MMF_NLM_SLOTS;
@@ -200,8 +227,26 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
         x[pol][i] = valid ? sx[e0 + pol * MMF_NLM_T + i] : make_double2(0.0, 0.0);
         if constexpr (NARR == 2 && MODE != NLM_ENTER) y[pol][i] = valid ? sy[e0 + pol * MMF_NLM_T + i] : make_double2(0.0, 0.0);
         if constexpr (MODE == NLM_S23) u[pol][i] = axpy(0.5, y[pol][i], x[pol][i]);
+        else if constexpr (MODE == NLM_AGR_ITJ) u[pol][i] = y[pol][i];   // |A|^2 at z + h: from the previous iterate
         else u[pol][i] = x[pol][i];
       }
+    if constexpr (MODE == NLM_AGR_IT1) {  // no contraction: Y <- exp(i T) X, element by element
+      if (valid) {
+        const double2 th = *reinterpret_cast<const double2*>(smem_raw + slot * slot_bytes + tab_off +
+                                                             (a * MMF_NLM_T + 2 * q) * sizeof(double));
+        double sn[2], cs[2];
+        sincos(th.x, &sn[0], &cs[0]);
+        sincos(th.y, &sn[1], &cs[1]);
+#pragma unroll
+        for (int pol = 0; pol < 2; ++pol)
+#pragma unroll
+          for (int i = 0; i < 2; ++i) sx[e0 + pol * MMF_NLM_T + i] = cmul(x[pol][i], make_double2(cs[i], sn[i]));
+      }
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&done[slot]);
+      continue;
+    }
     if constexpr (MODE == NLM_RK4) {
       cpx acc[2][2];
 #pragma unroll
@@ -244,7 +289,23 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
     nlm_contract<NK>(kf, P1, g, q, s[0], s[1]);
     const double g1[2] = {p.hg * s[0], p.hg * s[1]};
 
-    if constexpr (MODE == NLM_PLAIN || MODE == NLM_ENTER) {
+    if constexpr (MODE == NLM_AGR_S0 || MODE == NLM_AGR_ITJ) {
+      double2* tt = reinterpret_cast<double2*>(smem_raw + slot * slot_bytes + tab_off + (a * MMF_NLM_T + 2 * q) * sizeof(double));
+      if (valid) {
+        if constexpr (MODE == NLM_AGR_S0) {
+          *tt = make_double2(g1[0], g1[1]);   // T = h gamma S(A(z))
+        } else {
+          const double2 t0 = *tt;
+          double sn[2], cs[2];
+          sincos(0.5 * (t0.x + g1[0]), &sn[0], &cs[0]);   // (h gamma / 2) [S(A(z)) + S(A_{j-1}(z + h))]
+          sincos(0.5 * (t0.y + g1[1]), &sn[1], &cs[1]);
+#pragma unroll
+          for (int pol = 0; pol < 2; ++pol)
+#pragma unroll
+            for (int i = 0; i < 2; ++i) sy[e0 + pol * MMF_NLM_T + i] = cmul(x[pol][i], make_double2(cs[i], sn[i]));
+        }
+      }
+    } else if constexpr (MODE == NLM_PLAIN || MODE == NLM_ENTER) {
       cpx* so = (MODE == NLM_ENTER) ? sy : sx;  // ENTER keeps the field in the first array of the slot
       if (valid) {
 #pragma unroll

@@ -238,6 +238,16 @@ def test_cfg4_timed_plan_ssfm_every_element_50_steps(mmf, torch, orc):
     assert err.max() <= TOL_FIELD, (err.max(), err.argmax(), dmax)
 
 
+def test_cfg4_timed_plan_agrawal_every_element_50_steps(mmf, torch, orc):
+    p, ps, small, X = tiled_cfg4(torch, scale=2.0)
+    pl = plan_for(mmf, p)
+    pl.propagate_ssfm_agrawal(X, p.steps, niter=2)
+    torch.cuda.synchronize()
+    want = orc.ssfm_agrawal(small, ps.dt, ps.h, ps.alpha, ps.beta, ps.gamma, ps.kappa, p.steps, niter=2)
+    err, dmax = tiled_error(torch, X, want)
+    assert err.max() <= TOL_FIELD, (err.max(), err.argmax(), dmax)
+
+
 # -------------------------------------------------------- configs 2 and 3 at FULL size and FULL step count (golden)
 # The oracle needs ~30-45 min per config for these, so its output is stored, sampled, by tests/golden/make_golden.py
 # (a committed script that calls only oracle/ and workloads.py; its header has the command).

@@ -79,3 +79,41 @@ def test_ssfm_cfg4_full_no_dispersion_sampled_samples(mmf, torch, orc):
     want = orc.ssfm_rk4(sub, p.dt, p.h, 0.0, np.zeros_like(p.beta), p.gamma, p.kappa, 2)
     assert workloads.rel_l2_per_field(want, sub).min() > 1e-3
     assert workloads.rel_l2_per_field(got, want).max() <= TOL_FIELD
+
+
+# ---------------------------------------------------------------------------------------------------- SSFM-Agrawal
+AGR_CASES = [(0, 2, 12, 100, 2), (1, 6, 13, 20, 2), (1, 6, 16, 6, 3), (2, 36, 14, 5, 2), (3, 120, 13, 3, 2),
+             (4, 7, 18, 3, 1), (4, 1, 4, 3, 2), (3, 120, 18, 2, 2), (0, 5, 9, 7, 4)]
+
+
+@pytest.mark.parametrize("cfg,M,logn,steps,niter", AGR_CASES)
+def test_agrawal_matches_oracle(mmf, torch, orc, cfg, M, logn, steps, niter):
+    """mmf_propagate_ssfm_agrawal against the oracle's ssfm_agrawal (odd and even step counts: the two field buffers
+    swap roles every step), relative L2 <= 1e-10 per field."""
+    p = workloads.problem(cfg, M=M, N=1 << logn, steps=steps)
+    A = p.field() * 3.0
+    pl = plan_for(mmf, p)
+    X = torch.from_numpy(A).to("cuda:0")
+    pl.propagate_ssfm_agrawal(X, steps, niter=niter)
+    torch.cuda.synchronize()
+    got = X.cpu().numpy()
+    want = orc.ssfm_agrawal(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, steps, niter=niter)
+    err = workloads.rel_l2_per_field(got, want)
+    assert workloads.rel_l2_per_field(want, A).min() > 1e-6
+    assert err.max() <= TOL_FIELD, (err.max(), err.argmax())
+
+
+def test_agrawal_composes_zero_steps_and_bad_arguments(mmf, torch):
+    import ctypes
+    p = workloads.problem(1, M=3, N=1 << 13, steps=5)
+    A = p.field()
+    pl = plan_for(mmf, p)
+    X = torch.from_numpy(A).to("cuda:0")
+    pl.propagate_ssfm_agrawal(X, 0)
+    assert np.array_equal(X.cpu().numpy(), A)
+    pl.propagate_ssfm_agrawal(X, 5)
+    Y = torch.from_numpy(A).to("cuda:0")
+    pl.propagate_ssfm_agrawal(Y, 2)
+    pl.propagate_ssfm_agrawal(Y, 3)
+    assert np.array_equal(Y.cpu().numpy(), X.cpu().numpy())
+    assert mmf.lib().mmf_propagate_ssfm_agrawal(pl._h, ctypes.c_void_p(X.data_ptr()), 1, 0, None) == mmf.MMF_EINVAL

@@ -107,3 +107,109 @@ def test_composition_and_zero_field(orc):
     assert np.array_equal(a, b)
     assert np.all(b[1] == 0) and np.any(b[0] != 0)
     assert np.array_equal(orc.ssfm_rk4(A, dt, h, 1e-3, beta, 0.5, kappa, 0), A)
+
+
+# ------------------------------------------------------------------------------------------------- SSFM-Agrawal
+# Symmetric split step with the iterative (trapezoidal) nonlinear part; reading R14.
+def agrawal_problem(seed=31, M=2, N=64):
+    rng = np.random.default_rng(seed)
+    X = np.zeros((2 * M, N), dtype=complex)
+    X[:, :5] = rand_c(rng, 2 * M, 5)
+    X[:, -4:] = rand_c(rng, 2 * M, 4)
+    A = np.fft.ifft(X, axis=1) * (N / 8)
+    beta = np.array([[0.0, 0.02, -0.06, 0.004], [0.0, -0.015, -0.04, -0.003]])[:M]
+    kappa = np.array([[1.0, 0.35], [0.8, 0.6]])[:M, :M]           # non-symmetric
+    return A, beta, kappa
+
+
+def test_agrawal_gamma_zero_is_the_exact_linear_solution(orc):
+    A, beta, kappa = agrawal_problem()
+    N, dt, h, steps, alpha = A.shape[1], 0.7, 3.0, 4, 0.02
+    w = 2 * np.pi * np.fft.fftfreq(N, d=dt)
+    want = np.empty_like(A)
+    for r in range(A.shape[0]):
+        want[r] = np.fft.ifft(np.exp(eq1_linear_symbol(w, alpha, beta[r // 2]) * h * steps) * np.fft.fft(A[r]))
+    for niter in (1, 2, 3):
+        assert rel(orc.ssfm_agrawal(A, dt, h, alpha, beta, 0.0, kappa, steps, niter=niter, nthreads=1), want) <= 1e-13
+
+
+def test_agrawal_no_dispersion_is_the_exact_phase_rotation_for_any_iteration_count(orc):
+    """alpha = beta = 0: a phase rotation conserves every |A_b|^2, so N(z+h) = N(z) and the trapezoid is exact —
+    one step of any size, any niter >= 1, gives A_a exp(i gamma sum_b kappa_ab P_b z) to rounding."""
+    M, N = 3, 32
+    rng = np.random.default_rng(23)
+    A = rand_c(rng, 2 * M, N) * np.array([1.0, 0.3, 0.7, 1.4, 0.2, 0.9])[:, None]
+    kappa = rng.uniform(0.1, 1.0, size=(M, M))                        # non-symmetric: catches a transposed kappa
+    gamma, z = 0.9, 1.7
+    S = kappa @ (np.abs(A[0::2]) ** 2 + np.abs(A[1::2]) ** 2)
+    want = A * np.exp(1j * gamma * np.repeat(S, 2, axis=0) * z)
+    for niter, steps in ((1, 1), (2, 1), (3, 4)):
+        got = orc.ssfm_agrawal(A, 1.0, z / steps, 0.0, np.zeros((M, 1)), gamma, kappa, steps, niter=niter, nthreads=1)
+        assert rel(got, want) <= 1e-13, (niter, steps)
+
+
+def test_agrawal_converged_iteration_is_time_reversible(orc):
+    """The fixed point of the iteration is the implicit trapezoidal split step A1 = D exp(i (h gamma/2)[S(A0) + S(A1)]) D A0,
+    which is symmetric in (A0, h) <-> (A1, -h): with alpha = 0 a step of +h followed by a step of -h returns the input
+    (to the iteration's convergence).  A nonlinear phase taken from the wrong field (D A(z) instead of A(z)), a missing
+    1/2, or a stale N(z+h) all break this at O(h^3); a single iteration (explicit) breaks it too."""
+    A, beta, kappa = agrawal_problem(seed=47)
+    dt, h, gamma = 1.0, 4.0, 0.05
+    fwd = orc.ssfm_agrawal(A, dt, h, 0.0, beta, gamma, kappa, 1, niter=40, nthreads=1)
+    back = orc.ssfm_agrawal(fwd, dt, -h, 0.0, beta, gamma, kappa, 1, niter=40, nthreads=1)
+    assert rel(fwd, A) > 1e-2
+    assert rel(back, A) <= 1e-12
+    fwd1 = orc.ssfm_agrawal(A, dt, h, 0.0, beta, gamma, kappa, 1, niter=1, nthreads=1)
+    back1 = orc.ssfm_agrawal(fwd1, dt, -h, 0.0, beta, gamma, kappa, 1, niter=1, nthreads=1)
+    assert rel(back1, A) > 1e-6
+    # the iterates converge geometrically to that fixed point
+    d = [rel(orc.ssfm_agrawal(A, dt, h, 0.0, beta, gamma, kappa, 1, niter=n, nthreads=1), fwd) for n in (1, 2, 3, 4)]
+    assert d[0] > d[1] > d[2] > d[3] and d[3] < 0.2 * d[1]
+
+
+def test_agrawal_second_order_global_error_against_independent_solution_of_eq1(orc):
+    from scipy.integrate import solve_ivp
+    M, N, dt, z = 2, 128, 1.0, 120.0
+    rng = np.random.default_rng(78)
+    X = np.zeros((2 * M, N), dtype=complex)
+    X[:, :4] = rand_c(rng, 2 * M, 4)
+    X[:, -3:] = rand_c(rng, 2 * M, 3)
+    A0 = np.fft.ifft(X, axis=1) * (N / 32) * np.array([9.0, 3.6, 6.6, 10.5])[:, None]
+    alpha, gamma = 2e-3, 1.7e-3
+    beta = np.array([[4e-3, 9e-3, -25e-3, 3e-3], [-6e-3, -7e-3, -18e-3, -2e-3]])
+    kappa = np.array([[1.0, 0.35], [0.8, 0.6]])
+    w = 2 * np.pi * np.fft.fftfreq(N, d=dt)
+    Lsym = np.vstack([eq1_linear_symbol(w, alpha, beta[r // 2]) for r in range(2 * M)])
+
+    def rhs(_z, y):
+        A = (y[: y.size // 2] + 1j * y[y.size // 2:]).reshape(2 * M, N)
+        lin = np.fft.ifft(Lsym * np.fft.fft(A, axis=1), axis=1)
+        P = np.abs(A[0::2]) ** 2 + np.abs(A[1::2]) ** 2
+        d = (lin + 1j * gamma * np.repeat(kappa @ P, 2, axis=0) * A).ravel()
+        return np.concatenate([d.real, d.imag])
+
+    y0 = np.concatenate([A0.ravel().real, A0.ravel().imag])
+    sol = solve_ivp(rhs, (0.0, z), y0, method="DOP853", rtol=1e-12, atol=1e-14)
+    assert sol.success
+    ref = (sol.y[: y0.size // 2, -1] + 1j * sol.y[y0.size // 2:, -1]).reshape(2 * M, N)
+    for niter in (2, 3):
+        errs = [rel(orc.ssfm_agrawal(A0, dt, z / n, alpha, beta, gamma, kappa, n, niter=niter, nthreads=1), ref)
+                for n in (32, 64, 128, 256)]
+        ratios = [errs[i] / errs[i + 1] for i in range(3)]
+        assert errs[-1] < 1e-3, errs
+        assert all(3.5 < r < 4.5 for r in ratios), (niter, errs, ratios)      # "a global error of O(h^2)" (PAPER.md:63)
+
+
+def test_agrawal_composition_and_zero_field(orc):
+    M, N, dt, h = 2, 32, 1.0, 2.0
+    rng = np.random.default_rng(6)
+    A = rand_c(rng, 2 * M, N) * 0.3
+    A[1] = 0
+    beta = np.array([[0.0, 0.01, -0.02, 0.001], [0.0, -0.01, -0.03, 0.001]])
+    kappa = np.array([[1.0, 0.4], [0.4, 1.0]])
+    a = orc.ssfm_agrawal(orc.ssfm_agrawal(A, dt, h, 1e-3, beta, 0.5, kappa, 2, nthreads=1), dt, h, 1e-3, beta, 0.5,
+                         kappa, 3, nthreads=1)
+    b = orc.ssfm_agrawal(A, dt, h, 1e-3, beta, 0.5, kappa, 5, nthreads=1)
+    assert np.array_equal(a, b)
+    assert np.all(b[1] == 0) and np.any(b[0] != 0)
+    assert np.array_equal(orc.ssfm_agrawal(A, dt, h, 1e-3, beta, 0.5, kappa, 0), A)
