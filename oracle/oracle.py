@@ -41,9 +41,11 @@ def lib():
         L.orc_nonlinear.argtypes = [dp, dp, i, ll, d, dp, i]
         L.orc_rk4ip.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
         L.orc_ssfm_rk4.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
+        L.orc_nonlinear_general.argtypes = [dp, dp, i, ll, d, dp, i]
+        L.orc_rk4ip_general.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
         L.orc_ssfm_agrawal.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i, i]
         for f in (L.orc_dft, L.orc_fft, L.orc_omega, L.orc_linear_table, L.orc_apply_D, L.orc_nonlinear,
-                  L.orc_rk4ip, L.orc_ssfm_rk4, L.orc_ssfm_agrawal):
+                  L.orc_rk4ip, L.orc_ssfm_rk4, L.orc_ssfm_agrawal, L.orc_nonlinear_general, L.orc_rk4ip_general):
             f.restype = i
         _lib = L
     return _lib
@@ -154,4 +156,29 @@ def ssfm_agrawal(A, dt, h, alpha, beta, gamma, kappa, nsteps, niter=2, nthreads=
     rc = lib().orc_ssfm_agrawal(_p(A), M, N, dt, h, alpha, _p(beta), beta.shape[1], gamma, _p(kappa), nsteps, niter,
                                 nthreads)
     assert rc == 0, "orc_ssfm_agrawal rejected its arguments"
+    return A
+
+
+def nonlinear_general(u, hgamma, kappa2, nthreads=1):
+    """(i hgamma sum_s kappa2[r][s] |u_s|^2) u_r with the general per-polarisation [2M][2M] coupling matrix."""
+    u = _c128(u)
+    R, N = u.shape
+    kappa2 = _f64(kappa2).reshape(R, R)
+    out = np.empty_like(u)
+    assert lib().orc_nonlinear_general(_p(u), _p(out), R // 2, N, hgamma, _p(kappa2), nthreads) == 0
+    return out
+
+
+def rk4ip_general(A, dt, h, alpha, beta, gamma, kappa2, nsteps, nthreads=None):
+    """rk4ip with kappa2: (2M, 2M), one coefficient per pair of polarisation modes."""
+    A = _c128(A).copy()
+    R, N = A.shape
+    M = R // 2
+    assert R == 2 * M
+    beta = _f64(beta).reshape(M, -1)
+    kappa2 = _f64(kappa2).reshape(R, R)
+    if nthreads is None:
+        nthreads = default_threads()
+    rc = lib().orc_rk4ip_general(_p(A), M, N, dt, h, alpha, _p(beta), beta.shape[1], gamma, _p(kappa2), nsteps, nthreads)
+    assert rc == 0, "orc_rk4ip_general rejected its arguments"
     return A

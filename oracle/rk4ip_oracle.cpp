@@ -202,27 +202,61 @@ void nonlinear(const cplx* u, cplx* out, int M, long long N, double hgamma, cons
   });
 }
 
+// The paper's own data structure (Fig. 2): one coupling coefficient per PAIR OF POLARISATION MODES,
+// "a matrix of 2M x 2M elements".  Row r = 2a + p of the field is polarisation mode r:
+//   out_r[t] = (i * hgamma * S_r[t]) * u_r[t],   S_r[t] = sum_{s=0}^{2M-1} kappa2[r][s] |u_s[t]|^2      (s ascending)
+// The Manakov form of nonlinear() is the special case kappa2[2a+p][2b+q] = kappa_ab.
+void nonlinear_general(const cplx* u, cplx* out, int M, long long N, double hgamma, const double* kappa2, int nthreads) {
+  const long long BLK = 4096;
+  const int R = 2 * M;
+  long long nblk = (N + BLK - 1) / BLK;
+  parallel_for(nblk, nthreads, [&](long long blk) {
+    std::vector<double> P(R);
+    long long t0 = blk * BLK, t1 = std::min(N, t0 + BLK);
+    for (long long t = t0; t < t1; ++t) {
+      for (int s = 0; s < R; ++s) {
+        cplx v = u[(long long)s * N + t];
+        P[s] = v.real() * v.real() + v.imag() * v.imag();
+      }
+      for (int r = 0; r < R; ++r) {
+        double S = 0.0;
+        for (int s = 0; s < R; ++s) S += kappa2[(long long)r * R + s] * P[s];
+        double g = hgamma * S;
+        cplx v = u[(long long)r * N + t];
+        out[(long long)r * N + t] = cplx(-g * v.imag(), g * v.real());  // (i g) * v
+      }
+    }
+  });
+}
+
+// N of Eq. (1) in either form: kappa is [M][M] (Manakov, general = false) or [2M][2M] (general = true)
+void apply_N(const cplx* u, cplx* out, int M, long long N, double hgamma, const double* kappa, bool general,
+             int nthreads) {
+  if (general) nonlinear_general(u, out, M, N, hgamma, kappa, nthreads);
+  else nonlinear(u, out, M, N, hgamma, kappa, nthreads);
+}
+
 // One RK4IP step, Eq. (6a)-(6f) in the paper's order and notation (R3, R4).
 // E is the table for hh = h/2.  Seven full-size buffers, nothing fused or reordered.
-void rk4ip_step(cplx* A, int M, long long N, const cplx* E, double hgamma, const double* kappa, int nthreads,
-                cplx* AI, cplx* k1, cplx* k2, cplx* k3, cplx* k4, cplx* tmp) {
+void rk4ip_step(cplx* A, int M, long long N, const cplx* E, double hgamma, const double* kappa, bool general,
+                int nthreads, cplx* AI, cplx* k1, cplx* k2, cplx* k3, cplx* k4, cplx* tmp) {
   const long long tot = 2LL * M * N;
   // (6a) A_I = exp(h/2 L) A
   std::memcpy((void*)AI, (const void*)A, sizeof(cplx) * tot);
   apply_D(AI, M, N, E, nthreads);
   // (6b) k1 = exp(h/2 L) [ h N(A) A ]
-  nonlinear(A, k1, M, N, hgamma, kappa, nthreads);
+  apply_N(A, k1, M, N, hgamma, kappa, general, nthreads);
   apply_D(k1, M, N, E, nthreads);
   // (6c) k2 = h N(A_I + k1/2) [A_I + k1/2]
   for (long long i = 0; i < tot; ++i) tmp[i] = AI[i] + k1[i] / 2.0;
-  nonlinear(tmp, k2, M, N, hgamma, kappa, nthreads);
+  apply_N(tmp, k2, M, N, hgamma, kappa, general, nthreads);
   // (6d) k3 = h N(A_I + k2/2) [A_I + k2/2]
   for (long long i = 0; i < tot; ++i) tmp[i] = AI[i] + k2[i] / 2.0;
-  nonlinear(tmp, k3, M, N, hgamma, kappa, nthreads);
+  apply_N(tmp, k3, M, N, hgamma, kappa, general, nthreads);
   // (6e) k4 = h N( exp(h/2 L)[A_I + k3] ) exp(h/2 L)[A_I + k3]
   for (long long i = 0; i < tot; ++i) tmp[i] = AI[i] + k3[i];
   apply_D(tmp, M, N, E, nthreads);
-  nonlinear(tmp, k4, M, N, hgamma, kappa, nthreads);
+  apply_N(tmp, k4, M, N, hgamma, kappa, general, nthreads);
   // (6f) A(z+h) = exp(h/2 L)[A_I + k1/6 + k2/3 + k3/3] + k4/6
   for (long long i = 0; i < tot; ++i) tmp[i] = AI[i] + k1[i] / 6.0 + k2[i] / 3.0 + k3[i] / 3.0;
   apply_D(tmp, M, N, E, nthreads);
@@ -354,7 +388,29 @@ int orc_rk4ip(double* A, int M, long long N, double dt, double h, double alpha, 
   std::vector<cplx> E((size_t)M * N), AI(tot), k1(tot), k2(tot), k3(tot), k4(tot), tmp(tot);
   linear_table(E.data(), M, N, dt, h / 2.0, alpha, beta, K, nthreads);
   for (int s = 0; s < nsteps; ++s)
-    rk4ip_step((cplx*)A, M, N, E.data(), h * gamma, kappa, nthreads, AI.data(), k1.data(), k2.data(), k3.data(),
+    rk4ip_step((cplx*)A, M, N, E.data(), h * gamma, kappa, false, nthreads, AI.data(), k1.data(), k2.data(), k3.data(),
+               k4.data(), tmp.data());
+  return 0;
+}
+
+// out[2M][N] = (i * hgamma * sum_s kappa2[r][s] |u_s|^2) * u_r;  kappa2 is [2M][2M] row-major.
+int orc_nonlinear_general(const double* u, double* out, int M, long long N, double hgamma, const double* kappa2,
+                          int nthreads) {
+  if (!u || !out || !kappa2 || M < 1 || N < 1) return -1;
+  nonlinear_general((const cplx*)u, (cplx*)out, M, N, hgamma, kappa2, nthreads);
+  return 0;
+}
+
+// orc_rk4ip with the general per-polarisation coupling matrix kappa2 [2M][2M].
+int orc_rk4ip_general(double* A, int M, long long N, double dt, double h, double alpha, const double* beta, int K,
+                      double gamma, const double* kappa2, int nsteps, int nthreads) {
+  if (!A || !beta || !kappa2 || M < 1 || K < 1 || !is_pow2(N) || !(dt > 0) || nsteps < 0) return -1;
+  if (nsteps == 0) return 0;
+  const long long tot = 2LL * M * N;
+  std::vector<cplx> E((size_t)M * N), AI(tot), k1(tot), k2(tot), k3(tot), k4(tot), tmp(tot);
+  linear_table(E.data(), M, N, dt, h / 2.0, alpha, beta, K, nthreads);
+  for (int s = 0; s < nsteps; ++s)
+    rk4ip_step((cplx*)A, M, N, E.data(), h * gamma, kappa2, true, nthreads, AI.data(), k1.data(), k2.data(), k3.data(),
                k4.data(), tmp.data());
   return 0;
 }

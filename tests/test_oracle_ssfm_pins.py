@@ -213,3 +213,37 @@ def test_agrawal_composition_and_zero_field(orc):
     assert np.array_equal(a, b)
     assert np.all(b[1] == 0) and np.any(b[0] != 0)
     assert np.array_equal(orc.ssfm_agrawal(A, dt, h, 1e-3, beta, 0.5, kappa, 0), A)
+
+
+# ------------------------------------------------------------------------ the step-size claim
+def test_stepsize_table_claim(orc):
+    """tests/golden/stepsize_table.md (written by tests/golden/make_stepsize_table.py from the oracle alone): one row
+    is re-derived here with a coarser reference, and the table must show what the paper states — RK4IP reaches a given
+    accuracy with more than twice the step size of the split-step schemes, and the orders are 4 / 2 / 2."""
+    import importlib.util
+    import os
+    import re
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_stepsize_table", os.path.join(here, "make_stepsize_table.py"))
+    mk = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mk)
+    rows = {}
+    for line in open(os.path.join(here, "stepsize_table.md")):
+        m = re.match(r"\| ([0-9.]+) \| (\d+) \| ([0-9.e+-]+) \| ([0-9.e+-]+) \| ([0-9.e+-]+) \|", line)
+        if m:
+            rows[int(m.group(2))] = [float(m.group(i)) for i in (3, 4, 5)]
+    assert sorted(rows) == list(mk.STEPS)
+    p, A = mk.setup()
+    ref = mk.reference(p, A, n=1280)
+    got = mk.errors(p, A, ref, 80)
+    for name, want in zip(got, rows[80]):
+        assert abs(got[name] / want - 1.0) < 0.02, (name, got[name], want)
+    hs = [mk.LENGTH_M / n for n in mk.STEPS]
+    for target in (1e-3, 1e-4):
+        h_ip, h_rk, _ = (mk.step_for_accuracy(hs, [rows[n][c] for n in mk.STEPS], target) for c in range(3))
+        assert h_ip / h_rk > 2.0, (target, h_ip, h_rk)
+    h_ip = mk.step_for_accuracy(hs, [rows[n][0] for n in mk.STEPS], 1e-3)
+    h_ag = mk.step_for_accuracy(hs, [rows[n][2] for n in mk.STEPS], 1e-3)
+    assert h_ip / h_ag > 2.0
+    order = lambda c: math.log2(rows[160][c] / rows[320][c])
+    assert 3.7 < order(0) < 4.7 and 1.8 < order(1) < 2.2 and 1.8 < order(2) < 2.2
