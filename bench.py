@@ -57,6 +57,21 @@ def load_peaks():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def load_fp64_peak(sms):
+    """fp64 peak [TFLOP/s]: the best DFMA / DMMA rate `bench.py --probes` measured (newest profiles/r*_probes.json),
+    else derived: 64 DFMA per clock per SM x 2 flop x SM count x 1.965 GHz."""
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_probes.json")))
+    if files:
+        try:
+            with open(files[-1]) as f:
+                d = json.load(f)
+            return max(e["TFLOP_s"] for e in d["probes"]["fp64"]), "measured (%s)" % os.path.relpath(files[-1], ROOT)
+        except Exception:
+            pass
+    return 64 * 2 * sms * 1.965e9 / 1e12, "derived (64 DFMA/clk/SM x SMs x 1.965 GHz)"
+
+
 def workload_string(p):
     return ("cfg%d: M=%d modes x 2 pol, N=2^%d fp64 complex, dt=%g ps, h=%g m, K=4 beta terms, kappa %dx%d; "
             "input: %s" % (p.cfg, p.M, p.N.bit_length() - 1, p.dt, p.h, p.M, p.M, p._c["signal"]))
@@ -317,7 +332,9 @@ def run_mmf(args):
     if world > 1:                                    # replicas: a launch-power sweep, one power per rank
         X *= replicas.amplitude_scale(rank, world)
         H.copy_(X)
-    plan = binding.Plan(p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, device=dev)
+    general = args.kappa == "general"
+    plan = binding.Plan(p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa_general() if general else p.kappa,
+                        device=dev, general=general)
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -332,7 +349,11 @@ def run_mmf(args):
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    plan.set_timing(True)
+    # Per-launch CUDA events bracket every kernel of the timed region (the roofline's launch durations) — except for
+    # the small configs, whose step body replays from a CUDA graph (mmf_api.cu): there the events would force the
+    # launch-by-launch path and slow the very thing being measured, so the breakdown comes from a second, untimed pass.
+    events_in_region = F > (64 << 20)
+    plan.set_timing(events_in_region)
     n0 = plan.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -342,32 +363,61 @@ def run_mmf(args):
     barrier()
     launches = plan.launch_count() - n0
     ms = e0.elapsed_time(e1)
+    if not events_in_region:
+        plan.set_timing(True)
+        advance(X, min(args.steps, 20))
+        torch.cuda.synchronize()
     kern = plan.get_timing()
     plan.set_timing(False)
     clocks = sampler.stop()
     _, ms, value = replicas.whole_job(p.R * p.N * args.steps, ms, dist, dev)
     assert bool(torch.isfinite(X.view(torch.float64)).all()), "propagated field is not finite"
 
-    # ---- end to end: host buffer in, host buffer out, through the C ABI ----
+    # ---- end to end: host buffers in, host buffers out, through the C ABI ----
+    # (a) one field per call (mmf_propagate_host): H2D, K steps, D2H, all serial — one field cannot hide its copies;
+    # (b) a stream of B fields per call (mmf_propagate_host_batch, e.g. a launch-power sweep): field i + 1 goes in and
+    #     field i - 1 comes out while field i propagates.  (b) is the throughput figure; (a) is reported beside it.
     barrier()
     e0.record(stream)
     if args.method == "rk4ip":
         plan.propagate_host(H, X, args.steps)       # H2D copy, K steps, D2H copy, stream synchronised inside
-    else:                                           # no host entry point for the split step: same copies by hand
+    else:                                           # no host entry point for the split steps: same copies by hand
         X.copy_(H, non_blocking=True)
         advance(X, args.steps)
         H.copy_(X, non_blocking=True)
     e1.record(stream)
     barrier()
-    ms_e2e = e0.elapsed_time(e1)                    # device clock over the whole call
-    _, ms_e2e, e2e_value = replicas.whole_job(p.R * p.N * args.steps, ms_e2e, dist, dev)
+    ms_single = e0.elapsed_time(e1)                 # device clock over the whole call
+    _, ms_single, single_value = replicas.whole_job(p.R * p.N * args.steps, ms_single, dist, dev)
+    nbatch, ms_e2e, e2e_value = 1, ms_single, single_value
+    if args.method == "rk4ip" and args.e2e_batch > 1:
+        _, avail = host_description()
+        free_dev = torch.cuda.mem_get_info(dev)[0]
+        nbatch = args.e2e_batch
+        while nbatch > 1 and ((avail or 0) * 2 ** 30 < (nbatch - 1) * F * world + (16 << 30)):
+            nbatch -= 1
+        if free_dev < F + (2 << 30):
+            nbatch = 1
+        if nbatch > 1:
+            hosts = [H] + [torch.empty((p.R, p.N), dtype=torch.complex128, pin_memory=True) for _ in range(nbatch - 1)]
+            for Hx in hosts[1:]:
+                Hx.copy_(H)
+            X2 = torch.empty_like(X)
+            barrier()
+            e0.record(stream)
+            plan.propagate_host_batch(hosts, X, X2, args.steps)
+            e1.record(stream)
+            barrier()
+            ms_e2e = e0.elapsed_time(e1)
+            _, ms_e2e, e2e_value = replicas.whole_job(nbatch * p.R * p.N * args.steps, ms_e2e, dist, dev)
+            del X2, hosts
 
     if rank != 0:
         return 0
 
     # ---- roofline of the dominant kernel (largest summed device time in the timed region) ----
     peak, peak_src = load_peaks()
-    full_cfg = args.modes is None and args.logn is None and args.method == "rk4ip"
+    full_cfg = args.modes is None and args.logn is None and args.method == "rk4ip" and not general
     roof = None
     breakdown = []
     tot_kernel_ms = sum(k["total_ms"] for k in kern) or 1.0
@@ -397,6 +447,21 @@ def run_mmf(args):
                                   "achieved_Tinst_s": ctr["fp64_thread_inst"] / (avg * 1e-3) / 1e12,
                                   "peak_Tinst_s": peak_i / 1e12, "frac": ctr["fp64_thread_inst"] / (avg * 1e-3) / peak_i,
                                   "sm_mhz": clk / 1e6}
+    fp64_peak, fp64_src = load_fp64_peak(torch.cuda.get_device_properties(dev).multi_processor_count)
+    if general and kern:
+        # the general contraction is 2 (2M)^2 flop per sample per evaluation: its kernels are bound by the fp64 (tensor)
+        # pipe, so the dominant one reports BOTH bounds ("report both bounds in roofline")
+        nlg = [k for k in kern if k["name"].startswith("k_nlg")]
+        if nlg:
+            topg = max(nlg, key=lambda k: k["total_ms"])
+            avg = topg["total_ms"] / topg["launches"]
+            flops = 2.0 * (2 * p.M) ** 2 * p.N
+            ach = flops / (avg * 1e-3) / 1e12
+            gb = topg["alg_bytes_per_launch"] / (avg * 1e-3) / 1e9
+            roof = {"bound": "alu", "kernel": topg["name"], "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s",
+                    "frac": ach / fp64_peak, "traffic": None, "peak_source": fp64_src, "flop_per_launch": flops,
+                    "avg_launch_ms": avg, "hbm": {"achieved": gb, "peak": peak, "unit": "GB/s", "frac": gb / peak,
+                                                  "alg_bytes_per_launch": topg["alg_bytes_per_launch"]}}
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
     if args.method == "rk4ip":
         balg = (36 if p.N > 4096 else 20) * F
@@ -406,6 +471,10 @@ def run_mmf(args):
         balg = (14 if p.N > 4096 else 6) * F
     t_roof_ms = balg / (peak * 1e9) * 1e3
     step_roof = {"B_alg_bytes_per_step": balg, "hbm_time_ms": t_roof_ms, "frac": t_roof_ms / (ms / args.steps)}
+    if general:   # the slower of the step's bytes at HBM bandwidth and its fp64 flops at peak (north_star)
+        t_alu_ms = 4 * 2.0 * (2 * p.M) ** 2 * p.N / (fp64_peak * 1e12) * 1e3
+        step_roof.update({"alu_time_ms": t_alu_ms, "fp64_peak_TFLOP_s": fp64_peak,
+                          "frac": max(t_roof_ms, t_alu_ms) / (ms / args.steps)})
     if args.method == "rk4ip" and p.N > 4096:      # this plan's own count: (6c)+(6d) in one pass -> 32 F
         step_roof["frac_of_32F_plan"] = (32 * F / (peak * 1e9) * 1e3) / (ms / args.steps)
 
@@ -451,13 +520,19 @@ def run_mmf(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_string(p), "method": args.method, "l2": "field copy %.1f GiB >> 126 MB L2 (no flush needed)"
+            "config": {"workload": workload_string(p) + (" [general 2M x 2M kappa]" if general else ""),
+                       "method": args.method, "kappa": args.kappa, "l2": "field copy %.1f GiB >> 126 MB L2 (no flush needed)"
                        % (F / 2 ** 30) if F > 4 * 126e6 else "working set near/below L2 size: L2-resident",
                        "parallelism": "replicas x%d (launch-power sweep, no collective)" % world},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": F / args.steps,
-                    "d2h_bytes_per_step": F / args.steps, "ms_per_call": ms_e2e,
-                    "call": "mmf_propagate_host(nsteps=%d): one H2D + one D2H of F per call" % args.steps},
+                    "d2h_bytes_per_step": F / args.steps, "ms_per_call": ms_e2e, "fields_per_call": nbatch,
+                    "call": ("mmf_propagate_host_batch(nfields=%d, nsteps=%d): every field one H2D + one D2H of F, copies of "
+                             "neighbouring fields overlap the propagation" % (nbatch, args.steps)) if nbatch > 1 else
+                            "mmf_propagate_host(nsteps=%d): one H2D + one D2H of F per call" % args.steps,
+                    "single_field_call": {"value": single_value, "ms_per_call": ms_single,
+                                          "call": "mmf_propagate_host(nsteps=%d): copies serial with the propagation"
+                                                  % args.steps}},
             "gpu_launches": launches, "roofline": roof, "step_roofline": step_roof, "kernels": breakdown, "cufft_reference": cufft,
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
@@ -477,11 +552,16 @@ def main():
                     help="rk4ip (Eq. 6, the headline path), ssfm (SSFM-RK4) or agrawal (SSFM-Agrawal): the symmetric "
                          "split step of Eq. 4 with a Runge-Kutta resp. an iterative nonlinear part")
     ap.add_argument("--niter", type=int, default=2, help="iterations per step of --method agrawal")
+    ap.add_argument("--kappa", default="manakov", choices=["manakov", "general"],
+                    help="manakov: kappa [M][M] of Eq. 1 (the headline path); general: the paper's [2M][2M] per-polarisation "
+                         "matrix (PAPER.md:176; rk4ip only)")
     ap.add_argument("--modes", type=int, default=None, help="override the config's mode count M (extra data points)")
     ap.add_argument("--logn", type=int, default=None, help="override the config's N = 2^logn (extra data points)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT reference point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--e2e-batch", type=int, default=3,
+                    help="host fields per mmf_propagate_host_batch call of the end-to-end leg (1: single-field call only)")
     ap.add_argument("--probes", action="store_true",
                     help="measure the fp64 issue peaks and the TMA access-pattern ceilings instead of the benchmark")
     args = ap.parse_args()

@@ -45,6 +45,15 @@ typedef struct mmf_plan mmf_plan; /* opaque */
 int mmf_plan_create(mmf_plan **out, int M, long long N, double dt, double h, double alpha, const double *beta, int K,
                     double gamma, const double *kappa);
 
+/* Same, with the GENERAL coupling matrix the paper's implementation stores (Fig. 2: "a matrix of
+ * 2M x 2M elements", one coefficient per pair of polarisation modes):
+ *   kappa2  host, [2M][2M] row-major, kappa2[r*2M + s] couples row s (= 2b + q) into row r (= 2a + p):
+ *           N_r = i gamma sum_s kappa2[r][s] |A_s|^2.  Need not be symmetric.  kappa2[2a+p][2b+q] = kappa_ab is Eq. (1).
+ * Requires M <= 120 (MMF_EINVAL otherwise).  Such a plan runs mmf_propagate, mmf_propagate_host and mmf_apply_*;
+ * the split-step entry points return MMF_EINVAL for it.  Workspace: three more field buffers (four when N > 4096). */
+int mmf_plan_create_general(mmf_plan **out, int M, long long N, double dt, double h, double alpha, const double *beta,
+                            int K, double gamma, const double *kappa2);
+
 /* Bytes of device workspace the plan needs: one more full-field buffer when N <= 4096, two when N > 4096 (three resp.
  * four when M > 120) plus the tabulated exp(h/2 L_a(w_k)) of Eq. (6a) (one row per mode), plus for N <= 4096 a real
  * [M][N] table for mmf_propagate_ssfm_agrawal.  The caller allocates it
@@ -61,6 +70,13 @@ int mmf_plan_set_workspace(mmf_plan *plan, void *ws_dev, size_t bytes, void *cud
  *   A_dev  device, [2M][N] complex128 (layout above), 16-byte aligned.  nsteps >= 0 (0 is a no-op).
  * Calling with n1 then n2 steps equals one call with n1+n2 steps. */
 int mmf_propagate(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
+
+/* A link of nspans fibre spans (section 6: "After each span, the fiber losses are compensated by a
+ * noiseless amplifier with flat-gain profile"): nspans x steps_per_span RK4IP steps, and after the last step of every
+ * span A <- gain * A (gain = AMPLITUDE factor, the same for all modes and frequencies; exp(alpha h steps_per_span / 2)
+ * compensates the span loss exactly).  The multiplication rides on the last kernel of the span: no extra pass.
+ * nspans >= 0, steps_per_span >= 1, gain finite.  Equals mmf_propagate(steps_per_span) + a scaling, nspans times. */
+int mmf_propagate_spans(mmf_plan *plan, void *A_dev, int nspans, int steps_per_span, double gain, void *cuda_stream);
 
 /* Advance A by nsteps SYMMETRIC SPLIT STEPS of size h with a Runge-Kutta nonlinear substep ("SSFM-RK4": Eq. 4
  * PAPER.md:58-61 with the nonlinear part solved by classical RK4), in place:
@@ -82,6 +98,15 @@ int mmf_propagate_ssfm_agrawal(mmf_plan *plan, void *A_dev, int nsteps, int nite
  * (device, [2M][N] complex128, caller-owned), propagates, copies back and SYNCHRONISES the stream.  A_host should be
  * page-locked for full copy bandwidth.  This is the end-to-end entry point bench.py times. */
 int mmf_propagate_host(mmf_plan *plan, void *A_host, void *A_dev_scratch, int nsteps, void *cuda_stream);
+
+/* A stream of nfields HOST fields through one plan (e.g. a launch-power sweep of one fibre): field i propagates on
+ * `cuda_stream` while field i + 1 is copied in and field i - 1 is copied out on two internal copy streams, over the two
+ * device buffers A_dev0 / A_dev1 (device, [2M][N] complex128 each, caller-owned; A_dev1 may be null when nfields == 1).
+ *   A_hosts  host array of nfields host pointers, each [2M][N] complex128, page-locked for the copies to overlap.
+ * Every field is advanced nsteps RK4IP steps in place (in its host buffer).  SYNCHRONISES before returning.
+ * (One field alone cannot hide its copies: the first transform of a step needs the whole time axis of every row.) */
+int mmf_propagate_host_batch(mmf_plan *plan, void *const *A_hosts, int nfields, void *A_dev0, void *A_dev1, int nsteps,
+                             void *cuda_stream);
 
 /* Stage-level entry points (each is a row group of the hot path; used by the parity tests).
  * mmf_apply_linear:    X <- exp(h/2 L) X  (Eq. 6a: transform, multiply by exp(h/2 L_a(w_k)), transform back), in place.

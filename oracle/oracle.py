@@ -43,9 +43,10 @@ def lib():
         L.orc_ssfm_rk4.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
         L.orc_nonlinear_general.argtypes = [dp, dp, i, ll, d, dp, i]
         L.orc_rk4ip_general.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
+        L.orc_rk4ip_spans.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i, i, d, i]
         L.orc_ssfm_agrawal.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i, i]
         for f in (L.orc_dft, L.orc_fft, L.orc_omega, L.orc_linear_table, L.orc_apply_D, L.orc_nonlinear,
-                  L.orc_rk4ip, L.orc_ssfm_rk4, L.orc_ssfm_agrawal, L.orc_nonlinear_general, L.orc_rk4ip_general):
+                  L.orc_rk4ip, L.orc_ssfm_rk4, L.orc_ssfm_agrawal, L.orc_nonlinear_general, L.orc_rk4ip_general, L.orc_rk4ip_spans):
             f.restype = i
         _lib = L
     return _lib
@@ -181,4 +182,20 @@ def rk4ip_general(A, dt, h, alpha, beta, gamma, kappa2, nsteps, nthreads=None):
         nthreads = default_threads()
     rc = lib().orc_rk4ip_general(_p(A), M, N, dt, h, alpha, _p(beta), beta.shape[1], gamma, _p(kappa2), nsteps, nthreads)
     assert rc == 0, "orc_rk4ip_general rejected its arguments"
+    return A
+
+
+def rk4ip_spans(A, dt, h, alpha, beta, gamma, kappa, nspans, steps_per_span, gain, general=False, nthreads=None):
+    """nspans spans of steps_per_span RK4IP steps, each followed by the lumped amplifier A <- gain * A."""
+    A = _c128(A).copy()
+    R, N = A.shape
+    M = R // 2
+    beta = _f64(beta).reshape(M, -1)
+    kd = R if general else M
+    kappa = _f64(kappa).reshape(kd, kd)
+    if nthreads is None:
+        nthreads = default_threads()
+    rc = lib().orc_rk4ip_spans(_p(A), M, N, dt, h, alpha, _p(beta), beta.shape[1], gamma, _p(kappa), int(general),
+                               nspans, steps_per_span, gain, nthreads)
+    assert rc == 0, "orc_rk4ip_spans rejected its arguments"
     return A

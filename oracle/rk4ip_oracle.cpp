@@ -393,6 +393,27 @@ int orc_rk4ip(double* A, int M, long long N, double dt, double h, double alpha, 
   return 0;
 }
 
+// A link of nspans fibre spans (section 6: "two 80 km spans ... After each span, the fiber losses are
+// compensated by a noiseless amplifier with flat-gain profile"): each span is steps_per_span RK4IP steps of size h,
+// followed by the lumped amplifier A <- gain * A (gain = the AMPLITUDE factor, the same for every mode and frequency;
+// exp(alpha L_span / 2) compensates the loss exactly).  general != 0: kappa is the [2M][2M] matrix.
+int orc_rk4ip_spans(double* A, int M, long long N, double dt, double h, double alpha, const double* beta, int K,
+                    double gamma, const double* kappa, int general, int nspans, int steps_per_span, double gain,
+                    int nthreads) {
+  if (!A || !beta || !kappa || M < 1 || K < 1 || !is_pow2(N) || !(dt > 0) || nspans < 0 || steps_per_span < 1) return -1;
+  const long long tot = 2LL * M * N;
+  std::vector<cplx> E((size_t)M * N), AI(tot), k1(tot), k2(tot), k3(tot), k4(tot), tmp(tot);
+  linear_table(E.data(), M, N, dt, h / 2.0, alpha, beta, K, nthreads);
+  cplx* a = (cplx*)A;
+  for (int sp = 0; sp < nspans; ++sp) {
+    for (int s = 0; s < steps_per_span; ++s)
+      rk4ip_step(a, M, N, E.data(), h * gamma, kappa, general != 0, nthreads, AI.data(), k1.data(), k2.data(), k3.data(),
+                 k4.data(), tmp.data());
+    for (long long i = 0; i < tot; ++i) a[i] *= gain;      // the lumped amplifier at the end of the span
+  }
+  return 0;
+}
+
 // out[2M][N] = (i * hgamma * sum_s kappa2[r][s] |u_s|^2) * u_r;  kappa2 is [2M][2M] row-major.
 int orc_nonlinear_general(const double* u, double* out, int M, long long N, double hgamma, const double* kappa2,
                           int nthreads) {

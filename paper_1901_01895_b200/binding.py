@@ -14,9 +14,9 @@ LIB_PATH = os.path.join(_HERE, "libmmf_b200.so")
 MMF_OK, MMF_EINVAL, MMF_ENOMEM, MMF_ECUDA = 0, -1, -2, -3
 
 # every symbol include/mmf.h declares (tests check that the built library exports all of them)
-SYMBOLS = ["mmf_plan_create", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate", "mmf_propagate_ssfm",
-           "mmf_propagate_ssfm_agrawal",
-           "mmf_propagate_host", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
+SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate", "mmf_propagate_ssfm",
+           "mmf_propagate_ssfm_agrawal", "mmf_propagate_spans",
+           "mmf_propagate_host", "mmf_propagate_host_batch", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
            "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_set_timing", "mmf_kernel_class_count",
            "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version",
            "mmf_probe_fp64", "mmf_probe_tma_copy"]
@@ -41,6 +41,8 @@ def lib():
     dp = ctypes.POINTER(ctypes.c_double)
     L.mmf_plan_create.argtypes = [ctypes.POINTER(vp), i, ll, d, d, d, dp, i, d, dp]
     L.mmf_plan_create.restype = i
+    L.mmf_plan_create_general.argtypes = [ctypes.POINTER(vp), i, ll, d, d, d, dp, i, d, dp]
+    L.mmf_plan_create_general.restype = i
     L.mmf_plan_workspace_bytes.argtypes = [vp]
     L.mmf_plan_workspace_bytes.restype = sz
     L.mmf_plan_set_workspace.argtypes = [vp, vp, sz, vp]
@@ -49,10 +51,14 @@ def lib():
     L.mmf_propagate.restype = i
     L.mmf_propagate_ssfm.argtypes = [vp, vp, i, vp]
     L.mmf_propagate_ssfm.restype = i
+    L.mmf_propagate_spans.argtypes = [vp, vp, i, i, d, vp]
+    L.mmf_propagate_spans.restype = i
     L.mmf_propagate_ssfm_agrawal.argtypes = [vp, vp, i, i, vp]
     L.mmf_propagate_ssfm_agrawal.restype = i
     L.mmf_propagate_host.argtypes = [vp, vp, vp, i, vp]
     L.mmf_propagate_host.restype = i
+    L.mmf_propagate_host_batch.argtypes = [vp, ctypes.POINTER(vp), i, vp, vp, i, vp]
+    L.mmf_propagate_host_batch.restype = i
     L.mmf_apply_linear.argtypes = [vp, vp, vp]
     L.mmf_apply_linear.restype = i
     L.mmf_apply_nonlinear.argtypes = [vp, vp, vp, vp]
@@ -100,18 +106,21 @@ def _stream_ptr(stream=None):
 class Plan:
     """mmf_plan_create / mmf_plan_set_workspace / mmf_propagate / mmf_plan_destroy with torch-owned buffers."""
 
-    def __init__(self, M, N, dt, h, alpha, beta, gamma, kappa, device="cuda:0"):
+    def __init__(self, M, N, dt, h, alpha, beta, gamma, kappa, device="cuda:0", general=False):
+        """general=True: kappa is the [2M][2M] per-polarisation matrix (mmf_plan_create_general)."""
         import torch
         L = lib()
         self.M, self.N = int(M), int(N)
         beta = np.ascontiguousarray(beta, dtype=np.float64).reshape(self.M, -1)
-        kappa = np.ascontiguousarray(kappa, dtype=np.float64).reshape(self.M, self.M)
+        kd = 2 * self.M if general else self.M
+        kappa = np.ascontiguousarray(kappa, dtype=np.float64).reshape(kd, kd)
         self._h = ctypes.c_void_p()
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         dp = ctypes.POINTER(ctypes.c_double)
-        rc = L.mmf_plan_create(ctypes.byref(self._h), self.M, self.N, float(dt), float(h), float(alpha),
-                               beta.ctypes.data_as(dp), beta.shape[1], float(gamma), kappa.ctypes.data_as(dp))
+        create = L.mmf_plan_create_general if general else L.mmf_plan_create
+        rc = create(ctypes.byref(self._h), self.M, self.N, float(dt), float(h), float(alpha),
+                    beta.ctypes.data_as(dp), beta.shape[1], float(gamma), kappa.ctypes.data_as(dp))
         _check(rc, "mmf_plan_create")
         nbytes = L.mmf_plan_workspace_bytes(self._h)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
@@ -133,6 +142,12 @@ class Plan:
         _check(lib().mmf_propagate(self._h, self._field_ptr(A), int(nsteps), _stream_ptr(stream)), "mmf_propagate")
         return A
 
+    def propagate_spans(self, A, nspans, steps_per_span, gain, stream=None):
+        """nspans spans of steps_per_span RK4IP steps, the lumped amplifier A <- gain * A after each span."""
+        _check(lib().mmf_propagate_spans(self._h, self._field_ptr(A), int(nspans), int(steps_per_span), float(gain),
+                                         _stream_ptr(stream)), "mmf_propagate_spans")
+        return A
+
     def propagate_ssfm(self, A, nsteps, stream=None):
         """In-place SSFM-RK4 propagation (symmetric split step, Eq. 4) of a CUDA complex128 tensor [2M, N]."""
         _check(lib().mmf_propagate_ssfm(self._h, self._field_ptr(A), int(nsteps), _stream_ptr(stream)),
@@ -151,6 +166,18 @@ class Plan:
         _check(lib().mmf_propagate_host(self._h, ctypes.c_void_p(A_host.data_ptr()), self._field_ptr(A_scratch),
                                         int(nsteps), _stream_ptr(stream)), "mmf_propagate_host")
         return A_host
+
+    def propagate_host_batch(self, hosts, scratch0, scratch1, nsteps, stream=None):
+        """hosts: list of pinned torch complex128 CPU tensors (2M, N); scratch0 / scratch1: CUDA tensors of that shape."""
+        import torch
+        for H in hosts:
+            assert (not H.is_cuda) and H.dtype == torch.complex128 and H.is_contiguous()
+            assert tuple(H.shape) == (2 * self.M, self.N)
+        arr = (ctypes.c_void_p * len(hosts))(*[H.data_ptr() for H in hosts])
+        _check(lib().mmf_propagate_host_batch(self._h, arr, len(hosts), self._field_ptr(scratch0),
+                                              self._field_ptr(scratch1) if scratch1 is not None else None, int(nsteps),
+                                              _stream_ptr(stream)), "mmf_propagate_host_batch")
+        return hosts
 
     def apply_linear(self, X, stream=None):
         _check(lib().mmf_apply_linear(self._h, self._field_ptr(X), _stream_ptr(stream)), "mmf_apply_linear")
@@ -203,14 +230,14 @@ class Plan:
             pass
 
 
-def raw_create(M, N, dt, h, alpha, beta, K, gamma, kappa):
-    """mmf_plan_create with raw arguments (for error-path tests).  Returns (status, handle)."""
+def raw_create(M, N, dt, h, alpha, beta, K, gamma, kappa, general=False):
+    """mmf_plan_create(_general) with raw arguments (for error-path tests).  Returns (status, handle)."""
     h_ = ctypes.c_void_p()
     dp = ctypes.POINTER(ctypes.c_double)
     b = None if beta is None else np.ascontiguousarray(beta, dtype=np.float64).ctypes.data_as(dp)
     k = None if kappa is None else np.ascontiguousarray(kappa, dtype=np.float64).ctypes.data_as(dp)
-    rc = lib().mmf_plan_create(ctypes.byref(h_), int(M), int(N), float(dt), float(h), float(alpha), b, int(K),
-                               float(gamma), k)
+    create = lib().mmf_plan_create_general if general else lib().mmf_plan_create
+    rc = create(ctypes.byref(h_), int(M), int(N), float(dt), float(h), float(alpha), b, int(K), float(gamma), k)
     return rc, h_
 
 

@@ -11,6 +11,7 @@
 #include "fft_kernels.cuh"
 #include "nl_tma.cuh"
 #include "nl_simt.cuh"
+#include "nl_general.cuh"
 
 using namespace mmf;
 
@@ -110,6 +111,7 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct mmf_plan {
   int M = 0, K = 0, logn = 0, logn1 = 0, logn2 = 0;
   int nlm_nk = -1;   // k-steps of the tensor-path nonlinear kernel; -1: M too large, legacy kernels (4 buffers)
+  bool general = false;  // kappa is the general [2M][2M] per-polarisation matrix (k_nlg, four-buffer plan)
   int num_sms = 148;
   int device = 0;    // the device the plan's tables live on; every call must be made with it current
   long long N = 0;
@@ -122,6 +124,18 @@ struct mmf_plan {
   size_t ws_bytes = 0, field_bytes = 0;
   cpx *Y = nullptr, *Z = nullptr, *W = nullptr, *V = nullptr, *E = nullptr;
   double* T = nullptr;  // N <= 4096: the table of mmf_propagate_ssfm_agrawal (workspace)
+  // launch plan: everything a launch needs besides its arguments is computed once per plan —
+  // tensor maps per (kind, buffer), the dynamic shared-memory attribute and the occupancy per kernel — and the step
+  // body of small problems is replayed from a captured CUDA graph
+  struct MapEntry { int kind; const void* base; int aux; CUtensorMap map; };
+  std::vector<MapEntry> map_cache;
+  std::vector<const void*> attr_done;
+  struct OccEntry { const void* kern; int threads; size_t smem; int occ; };
+  std::vector<OccEntry> occ_cache;
+  bool dry_run = false;              // launch helpers prepare (attributes, maps) but do not launch
+  cudaStream_t cap_stream = nullptr; // capture stream of the step-body graphs
+  struct GraphEntry { const void* X; const void* Y; int reps; long long nlaunch; cudaGraphExec_t exec; };
+  std::vector<GraphEntry> graphs;
   long long launches = 0;
   // optional per-launch CUDA-event timing (mmf_plan_set_timing): one (start, stop) pair per launch
   bool timing = false;
@@ -135,11 +149,12 @@ namespace {
 // ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
 enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
        KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_NLM_ENTER, KC_NLM_EXIT, KC_NLM_AGR_S0,
-       KC_NLM_AGR_IT1, KC_NLM_AGR_ITJ, KC_PERM, KC_COUNT };
+       KC_NLM_AGR_IT1, KC_NLM_AGR_ITJ, KC_PERM, KC_NLG_PLAIN, KC_NLG_STAGE2, KC_NLG_STAGE3, KC_NLG_FINAL, KC_COUNT };
 const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
                                         "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>", "k_nlm<plain>",
                                         "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>", "k_nlm<enter>",
-                                        "k_nlm<exit>", "k_nlm<agr_s0>", "k_nlm<agr_it1>", "k_nlm<agr_itj>", "k_perm"};
+                                        "k_nlm<exit>", "k_nlm<agr_s0>", "k_nlm<agr_it1>", "k_nlm<agr_itj>", "k_perm",
+                                        "k_nlg<plain>", "k_nlg<stage2>", "k_nlg<stage3>", "k_nlg<final>"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
 struct LaunchTimer {
@@ -209,7 +224,7 @@ int strided_tile_map(const void* base, cuuint64_t inner_cpx, cuuint64_t nrows_ou
 
 // BLOCKED order (fft_kernels.cuh), the column tile of passes A / C: pitch rows of WB complex values, rows x N2/WB x N1
 // of them; box = W adjacent columns x min(N1, 256) rows
-int blocked_cols_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+int blocked_cols_map_build(const mmf_plan* p, const void* base, CUtensorMap* map) {
   const int logw = MMF_TILE_LOG - p->logn1, logwb = block_logw(p->logn1);
   return strided_tile_map(base, 1ULL << logwb, ((cuuint64_t)(2 * p->M)) << (p->logn2 - logwb + p->logn1), logw,
                           p->logn1 > 8 ? 256u : (1u << p->logn1), map);
@@ -217,11 +232,80 @@ int blocked_cols_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
 
 // BLOCKED order, the chunk of pass B: pitch rows of one block (N1 WB complex values), rows x N2/WB of them;
 // box = the WB values of one (block, p1) x min(N2/WB, 256) blocks
-int blocked_rows_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+int blocked_rows_map_build(const mmf_plan* p, const void* base, CUtensorMap* map) {
   const int logwb = block_logw(p->logn1), lognb = p->logn2 - logwb;
   return strided_tile_map(base, 1ULL << (p->logn1 + logwb), ((cuuint64_t)(2 * p->M)) << lognb, logwb,
                           lognb > 8 ? 256u : (1u << lognb), map);
 }
+
+// ---- launch-plan caches --------------------------------------------------------------------------------------------
+enum { MAP_COLS = 0, MAP_ROWS, MAP_TILE, MAP_TABLE, MAP_NATURAL };
+int field_tile_map_build(const mmf_plan* p, const void* base, CUtensorMap* map, int boxrows);
+int table_tile_map_build(const mmf_plan* p, const void* base, CUtensorMap* map);
+
+// the tensor map of `kind` over the buffer at `base` (aux: box rows of MAP_TILE), encoded once per plan and buffer
+int cached_map(mmf_plan* p, int kind, const void* base, int aux, CUtensorMap* out) {
+  for (const auto& e : p->map_cache)
+    if (e.kind == kind && e.base == base && e.aux == aux) {
+      *out = e.map;
+      return MMF_OK;
+    }
+  mmf_plan::MapEntry e;
+  e.kind = kind; e.base = base; e.aux = aux;
+  int rc = MMF_EINVAL;
+  switch (kind) {
+    case MAP_COLS: rc = blocked_cols_map_build(p, base, &e.map); break;
+    case MAP_ROWS: rc = blocked_rows_map_build(p, base, &e.map); break;
+    case MAP_TILE: rc = field_tile_map_build(p, base, &e.map, aux); break;
+    case MAP_TABLE: rc = table_tile_map_build(p, base, &e.map); break;
+    case MAP_NATURAL: {
+      const int logwb = block_logw(p->logn1);
+      rc = strided_tile_map(base, 1ULL << p->logn2, ((cuuint64_t)(2 * p->M)) << p->logn1, logwb,
+                            1u << (MMF_TILE_LOG - logwb), &e.map);
+      break;
+    }
+    default: break;
+  }
+  if (rc != MMF_OK) return rc;
+  if (p->map_cache.size() >= 64) p->map_cache.erase(p->map_cache.begin());   // callers that cycle through many buffers
+  p->map_cache.push_back(e);
+  *out = e.map;
+  return MMF_OK;
+}
+int blocked_cols_map(mmf_plan* p, const void* base, CUtensorMap* map) { return cached_map(p, MAP_COLS, base, 0, map); }
+int blocked_rows_map(mmf_plan* p, const void* base, CUtensorMap* map) { return cached_map(p, MAP_ROWS, base, 0, map); }
+int field_tile_map(mmf_plan* p, const void* base, CUtensorMap* map, int boxrows = 0) {
+  return cached_map(p, MAP_TILE, base, boxrows, map);
+}
+int table_tile_map(mmf_plan* p, const void* base, CUtensorMap* map) { return cached_map(p, MAP_TABLE, base, 0, map); }
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize, once per plan and kernel
+template <class K>
+int ensure_smem(mmf_plan* p, K kern, size_t smem) {
+  const void* key = reinterpret_cast<const void*>(kern);
+  for (const void* k : p->attr_done)
+    if (k == key) return MMF_OK;
+  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  p->attr_done.push_back(key);
+  return MMF_OK;
+}
+template <class K>
+int cached_occupancy(mmf_plan* p, K kern, int threads, size_t smem, int* occ) {
+  const void* key = reinterpret_cast<const void*>(kern);
+  for (const auto& e : p->occ_cache)
+    if (e.kern == key && e.threads == threads && e.smem == smem) {
+      *occ = e.occ;
+      return MMF_OK;
+    }
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, kern, threads, smem));
+  p->occ_cache.push_back({key, threads, smem, *occ});
+  return MMF_OK;
+}
+#define MMF_ENSURE_SMEM(kern, smem)                          \
+  do {                                                       \
+    const int rc__ = ensure_smem(p, kern, smem);             \
+    if (rc__ != MMF_OK) return rc__;                         \
+  } while (0)
 
 // ---- launch helpers ----------------------------------------------------------------------------------------------
 template <int LOGN1, int DIR>
@@ -229,7 +313,7 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   constexpr size_t smem = cols_smem_bytes<LOGN1>();
   constexpr int LOGW = MMF_TILE_LOG - LOGN1;
   auto kern = k_cols<LOGN1, DIR, kGroups>;
-  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
+  MMF_ENSURE_SMEM(kern, smem);
   ColsParams q;
   q.twtab = p->d_tw1; q.ipt = p->d_ipt;
   q.logn2 = p->logn2; q.logwb = block_logw(LOGN1); q.nrows = 2 * p->M; q.nbuf = nbuf;
@@ -239,6 +323,7 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   if ((rc = blocked_cols_map(p, nbuf > 1 ? X1 : X0, &map1)) != MMF_OK) return rc;
   const long long tiles = ((long long)nbuf * 2 * p->M) << (p->logn2 - LOGW);
   long long grid = tiles < p->num_sms ? tiles : p->num_sms;
+  if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, DIR == 0 ? KC_COLS_FWD : KC_COLS_INV, 2 * nbuf, st);
   kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(map0, map1, q);
   p->launches++;
@@ -263,7 +348,7 @@ int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cpx* OUT, cudaStream_
   constexpr size_t smem = rows_smem_bytes<LOGN2>();
   constexpr int LOGB = MMF_TILE_LOG - LOGN2;
   auto kern = k_rows<LOGN2, MODE, SINGLE, kGroups>;
-  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
+  MMF_ENSURE_SMEM(kern, smem);
   RowsParams q;
   q.X0 = X0; q.X1 = nbuf > 1 ? X1 : X0; q.OUT = OUT; q.E = p->E; q.twtab = p->d_tw2;
   CUtensorMap map0, map1;
@@ -278,6 +363,7 @@ int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cpx* OUT, cudaStream_
   q.logn1 = p->logn1; q.nbuf = nbuf; q.M = p->M;
   const long long items = SINGLE ? ((q.nchunks + (1 << LOGB) - 1) >> LOGB) : ((long long)p->M << (p->logn1 - LOGB));
   long long grid = items < p->num_sms ? items : p->num_sms;
+  if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_ROWS, 2 * nbuf, st);
   kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(map0, map1, q);
   p->launches++;
@@ -320,17 +406,16 @@ template <int DIR>
 int launch_perm(mmf_plan* p, cpx* natural, cpx* blocked, cudaStream_t st) {
   constexpr size_t smem = 3 * (sizeof(cpx) << MMF_TILE_LOG) + 64;
   auto kern = k_perm<DIR>;
-  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  MMF_ENSURE_SMEM(kern, smem);
   const int logwb = block_logw(p->logn1);
   CUtensorMap mapn;  // natural order: memory rows of N2 values, box = one block's WB columns x 4096 / WB rows
   int rc;
-  if ((rc = strided_tile_map(natural, 1ULL << p->logn2, ((cuuint64_t)(2 * p->M)) << p->logn1, logwb,
-                             1u << (MMF_TILE_LOG - logwb), &mapn)) != MMF_OK)
-    return rc;
+  if ((rc = cached_map(p, MAP_NATURAL, natural, 0, &mapn)) != MMF_OK) return rc;
   PermParams q;
   q.blocked = blocked; q.logn1 = p->logn1; q.logn2 = p->logn2; q.logwb = logwb; q.nrows = 2 * p->M;
   const long long tiles = ((long long)2 * p->M) << (p->logn1 + p->logn2 - MMF_TILE_LOG);
   long long grid = tiles < p->num_sms ? tiles : p->num_sms;
+  if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_PERM, 2, st);
   kern<<<(unsigned)grid, 32, smem, st>>>(mapn, q);
   p->launches++;
@@ -343,17 +428,19 @@ int to_natural(mmf_plan* p, cpx* tiled, cpx* natural, cudaStream_t st) { return 
 size_t nl_smem_bytes(const mmf_plan* p) { return sizeof(double) * 2 * (size_t)p->M * MMF_NL_T; }
 
 template <int MODE>
-int launch_nl(mmf_plan* p, cpx* X, cpx* Y, cpx* Z, cpx* W, cudaStream_t st) {
+int launch_nl(mmf_plan* p, cpx* X, cpx* Y, cpx* Z, cpx* W, cudaStream_t st, double gain = 1.0) {
   auto kern = k_nl<MODE>;
   const size_t smem = nl_smem_bytes(p);
-  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
+  MMF_ENSURE_SMEM(kern, smem);
   NlParams q;
   q.X = X; q.Y = Y; q.Z = Z; q.W = W;
   q.kappa = p->d_kappa;
   q.hg = p->h * p->gamma;
+  q.gain = gain;
   q.M = p->M;
   q.N = p->N;
   const unsigned grid = (unsigned)((p->N + MMF_NL_T - 1) / MMF_NL_T);
+  if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_NL_PLAIN + MODE, MODE == NL_PLAIN ? 2 : MODE == NL_STAGE2 ? 3 : MODE == NL_STAGE3 ? 5 : MODE == NL_FINAL ? 3 : 4, st);
   kern<<<grid, MMF_NL_T * MMF_NL_WARPS, smem, st>>>(q);
   p->launches++;
@@ -372,7 +459,7 @@ int nlm_pick_nk(int M) {
 }
 
 // tensor map of a field buffer [2M][N] complex128 seen as doubles [2M][2N], box = (8 samples = 16 doubles) x 2M rows
-int field_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+int field_tile_map_build(const mmf_plan* p, const void* base, CUtensorMap* map, int boxrows) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) {
     snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled is unavailable");
@@ -380,7 +467,7 @@ int field_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
   }
   const cuuint64_t gdim[2] = {(cuuint64_t)(2 * p->N), (cuuint64_t)(2 * p->M)};
   const cuuint64_t gstride[1] = {(cuuint64_t)p->N * sizeof(cpx)};
-  const cuuint32_t box[2] = {2 * MMF_NLM_T, (cuuint32_t)(2 * p->M)};
+  const cuuint32_t box[2] = {2 * MMF_NLM_T, (cuuint32_t)(boxrows > 0 ? boxrows : 2 * p->M)};
   const cuuint32_t estr[2] = {1, 1};
   const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), gdim, gstride, box, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
@@ -393,7 +480,7 @@ int field_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
 }
 
 // tensor map of the real table T [M][N] doubles (the SSFM-Agrawal modes), box = 8 samples x M rows
-int table_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
+int table_tile_map_build(const mmf_plan* p, const void* base, CUtensorMap* map) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) {
     snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: cuTensorMapEncodeTiled is unavailable");
@@ -416,12 +503,13 @@ int table_tile_map(const mmf_plan* p, const void* base, CUtensorMap* map) {
 // PLAIN: A = U, B = OUT; ENTER: A = the caller's field (natural order), B = X, C = Y; EXIT: A = X, B = Y, C = the
 // caller's field; AGR_*: A = X, B = Y, C = the real table T; other modes: A = X, B = Y (C unused).
 template <int NK, int MODE>
-int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st) {
+int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st, double gain) {
   auto kern = k_nlt<NK, MODE>;
   constexpr int NARR = nlm_narr<MODE>();
   NltParams q;
   q.kappa = p->d_kappa;
   q.hg = p->h * p->gamma;
+  q.gain = gain;
   q.M = p->M;
   q.NW = (p->M + 7) / 8;
   q.ntiles = p->N / MMF_NLM_T;
@@ -436,14 +524,15 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st) {
   } else if ((rc = field_tile_map(p, C ? C : B, &mapC)) != MMF_OK) return rc;
   const size_t smem = nlt_smem_bytes(p->M, NK, NARR, nlm_has_table<MODE>());
   const int threads = 32 * (q.NW + 1);
-  CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device and cheap: no caching
+  MMF_ENSURE_SMEM(kern, smem);
   int occ = 1;
-  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
+  if ((rc = cached_occupancy(p, kern, threads, smem, &occ)) != MMF_OK) return rc;
   if (occ < 1) return MMF_EINVAL;
   long long grid = (long long)p->num_sms * occ;        // persistent: every resident CTA walks its own tile list
   if (grid > q.ntiles) grid = q.ntiles;
   constexpr double kFields = (MODE == NLM_PLAIN || MODE == NLM_RK4) ? 2 : (MODE == NLM_S23 || MODE == NLM_FINAL_NEXT) ? 4
                              : MODE == NLM_AGR_S0 ? 1.25 : MODE == NLM_AGR_IT1 ? 2.25 : MODE == NLM_AGR_ITJ ? 3.25 : 3;
+  if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_NLM_PLAIN + MODE, kFields, st);
   kern<<<(unsigned)grid, threads, smem, st>>>(mapA, mapB, mapC, q);
   p->launches++;
@@ -452,9 +541,9 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st) {
 }
 
 template <int MODE>
-int launch_nlm(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st, cpx* C = nullptr) {
+int launch_nlm(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st, cpx* C = nullptr, double gain = 1.0) {
   switch (p->nlm_nk) {
-#define MMF_NLM_CASE(NKV) case NKV: return launch_nlm_t<NKV, MODE>(p, A, B, C, st);
+#define MMF_NLM_CASE(NKV) case NKV: return launch_nlm_t<NKV, MODE>(p, A, B, C, st, gain);
     MMF_NLM_CASE(1) MMF_NLM_CASE(2) MMF_NLM_CASE(3) MMF_NLM_CASE(4) MMF_NLM_CASE(6) MMF_NLM_CASE(8) MMF_NLM_CASE(9)
     MMF_NLM_CASE(12) MMF_NLM_CASE(16) MMF_NLM_CASE(20) MMF_NLM_CASE(24) MMF_NLM_CASE(28) MMF_NLM_CASE(30)
     MMF_NLM_CASE(32)
@@ -469,6 +558,40 @@ bool on_plan_device(const mmf_plan* p) {
   return cudaGetDevice(&dev) == cudaSuccess && dev == p->device;
 }
 
+// ---- general per-polarisation coupling (k_nlg): F0 / F1 full-tile inputs, Hin own-rows input, Ho0 / Ho1 outputs ------
+template <int MODE>
+int launch_nlg(mmf_plan* p, const cpx* F0, const cpx* F1, const cpx* Hin, cpx* Ho0, cpx* Ho1, cudaStream_t st,
+               double gain = 1.0) {
+  auto kern = k_nlg<MODE>;
+  NlgParams q;
+  q.kappa2 = p->d_kappa;
+  q.hg = p->h * p->gamma;
+  q.gain = gain;
+  q.M = p->M;
+  q.NW = (p->M + 7) / 8;
+  q.nchunk = (2 * p->M + 15) / 16;
+  q.ntiles = p->N / MMF_NLM_T;
+  CUtensorMap mF0, mF1, mHin, mHo0, mHo1;
+  int rc;
+  if ((rc = field_tile_map(p, F0, &mF0)) != MMF_OK) return rc;
+  if ((rc = field_tile_map(p, F1 ? F1 : F0, &mF1)) != MMF_OK) return rc;
+  if ((rc = field_tile_map(p, Hin ? Hin : F0, &mHin, p->M)) != MMF_OK) return rc;
+  if ((rc = field_tile_map(p, Ho0, &mHo0, p->M)) != MMF_OK) return rc;
+  if ((rc = field_tile_map(p, Ho1 ? Ho1 : Ho0, &mHo1, p->M)) != MMF_OK) return rc;
+  const size_t smem = nlg_smem_bytes(p->M, q.nchunk, nlg_nfull<MODE>(), nlg_half_in<MODE>());
+  MMF_ENSURE_SMEM(kern, smem);
+  long long pairs = p->num_sms / 2;                      // persistent: CTA pairs (the two halves of the rows)
+  if (pairs > q.ntiles) pairs = q.ntiles;
+  if (pairs < 1) pairs = 1;
+  constexpr double kFields = MODE == NLG_PLAIN ? 2 : MODE == NLG_STAGE2 ? 3 : MODE == NLG_STAGE3 ? 5 : 3;
+  if (p->dry_run) return MMF_OK;
+  LaunchTimer lt(p, KC_NLG_PLAIN + MODE, kFields, st);
+  kern<<<(unsigned)(2 * pairs), 32 * (q.NW + 1), smem, st>>>(mF0, mF1, mHin, mHo0, mHo1, q);
+  p->launches++;
+  CU(cudaGetLastError());
+  return MMF_OK;
+}
+
 bool finite_all(const double* v, size_t n) {
   for (size_t i = 0; i < n; ++i)
     if (!std::isfinite(v[i])) return false;
@@ -477,6 +600,10 @@ bool finite_all(const double* v, size_t n) {
 
 void free_tables(mmf_plan* p) {
   clear_events(p);
+  for (auto& g : p->graphs) cudaGraphExecDestroy(g.exec);
+  p->graphs.clear();
+  if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
+  p->cap_stream = nullptr;
   cudaFree(p->d_kappa);
   cudaFree(p->d_tw1);
   cudaFree(p->d_tw2);
@@ -500,21 +627,37 @@ const char* mmf_status_string(int status) {
   }
 }
 
+static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, double h, double alpha, const double* beta,
+                            int K, double gamma, const double* kappa, bool general);
+
 int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, double alpha, const double* beta, int K,
                     double gamma, const double* kappa) {
+  return plan_create_impl(out, M, N, dt, h, alpha, beta, K, gamma, kappa, false);
+}
+
+int mmf_plan_create_general(mmf_plan** out, int M, long long N, double dt, double h, double alpha, const double* beta,
+                            int K, double gamma, const double* kappa2) {
+  return plan_create_impl(out, M, N, dt, h, alpha, beta, K, gamma, kappa2, true);
+}
+
+static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, double h, double alpha, const double* beta,
+                            int K, double gamma, const double* kappa, bool general) {
   if (!out) return MMF_EINVAL;
   *out = nullptr;
   if (!beta || !kappa || M < 1 || K < 1 || K > MMF_MAXK) return MMF_EINVAL;
   if (N < 16 || N > (1LL << 24) || (N & (N - 1)) != 0) return MMF_EINVAL;
   if (!(dt > 0) || !std::isfinite(dt) || !std::isfinite(h) || !std::isfinite(alpha) || !std::isfinite(gamma))
     return MMF_EINVAL;
-  if (!finite_all(beta, (size_t)M * K) || !finite_all(kappa, (size_t)M * M)) return MMF_EINVAL;
+  const size_t KD = general ? 2 * (size_t)M : (size_t)M;   // kappa is KD x KD
+  if (general && M > MMF_NLG_MAXM) return MMF_EINVAL;       // the general kernel keeps an M x 2M slab in tensor memory
+  if (!finite_all(beta, (size_t)M * K) || !finite_all(kappa, KD * KD)) return MMF_EINVAL;
   if (sizeof(double) * 2 * (size_t)M * MMF_NL_T > 227 * 1024) return MMF_EINVAL;  // mode-power tile must fit one SM
   mmf_plan* p = new (std::nothrow) mmf_plan;
   if (!p) return MMF_ENOMEM;
   p->M = M; p->K = K; p->N = N; p->dt = dt; p->h = h; p->alpha = alpha; p->gamma = gamma;
   p->beta.assign(beta, beta + (size_t)M * K);
-  p->kappa.assign(kappa, kappa + (size_t)M * M);
+  p->kappa.assign(kappa, kappa + KD * KD);
+  p->general = general;
   int logn = 0;
   while ((1LL << logn) < N) ++logn;
   p->logn = logn;
@@ -526,7 +669,7 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
   else if (logn <= 22) p->logn1 = 10;
   else p->logn1 = 12;
   p->logn2 = logn - p->logn1;
-  p->nlm_nk = (M <= MMF_NLM_MAXM) ? nlm_pick_nk(M) : -1;
+  p->nlm_nk = (!general && M <= MMF_NLM_MAXM) ? nlm_pick_nk(M) : -1;
   {
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) == cudaSuccess) p->device = dev;
@@ -535,9 +678,9 @@ int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, dou
   p->field_bytes = sizeof(cpx) * 2 * (size_t)M * (size_t)N;
   int rc = MMF_OK;
   do {
-    cudaError_t e = cudaMalloc((void**)&p->d_kappa, sizeof(double) * (size_t)M * M);
+    cudaError_t e = cudaMalloc((void**)&p->d_kappa, sizeof(double) * KD * KD);
     if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MMF_ENOMEM : cuda_fail(e); break; }
-    e = cudaMemcpy(p->d_kappa, kappa, sizeof(double) * (size_t)M * M, cudaMemcpyHostToDevice);
+    e = cudaMemcpy(p->d_kappa, kappa, sizeof(double) * KD * KD, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { rc = cuda_fail(e); break; }
     if ((rc = upload_stage_tables(&p->d_tw2, p->logn2)) != MMF_OK) break;
     if (p->logn1 > 0) {
@@ -637,10 +780,93 @@ int mmf_plan_set_workspace(mmf_plan* p, void* ws_dev, size_t bytes, void* cuda_s
   return MMF_OK;
 }
 
-int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
+namespace {
+
+// one interior RK4IP step of the tensor-path plan: D(X,Y); S23; D(X,Y); FINAL_NEXT  (Eq. 6a-6f + the next 6b bracket)
+int step_body(mmf_plan* p, cpx* X, cpx* Y, cudaStream_t st, double gain = 1.0) {
+  int rc;
+  if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;
+  if ((rc = launch_nlm<NLM_S23>(p, X, Y, st)) != MMF_OK) return rc;
+  if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;
+  return launch_nlm<NLM_FINAL_NEXT>(p, X, Y, st, nullptr, gain);
+}
+
+// Small problems are bound by launch latency (hard part 6): their step body is captured once per
+// (X, Y, reps) into a CUDA graph and replayed.  Large ones gain nothing and launch directly.
+constexpr size_t kGraphMaxFieldBytes = (size_t)64 << 20;
+constexpr int kGraphReps = 16;
+
+cudaGraphExec_t body_graph(mmf_plan* p, cpx* X, cpx* Y, int reps, long long* nlaunch) {
+  for (const auto& g : p->graphs)
+    if (g.X == X && g.Y == Y && g.reps == reps) {
+      *nlaunch = g.nlaunch;
+      return g.exec;
+    }
+  if (!p->cap_stream && cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    p->cap_stream = nullptr;
+    return nullptr;
+  }
+  p->dry_run = true;   // attributes, occupancy and tensor maps: everything that is not a stream operation, up front
+  int rc = step_body(p, X, Y, p->cap_stream);
+  p->dry_run = false;
+  if (rc != MMF_OK) return nullptr;
+  const long long before = p->launches;
+  if (cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  for (int i = 0; i < reps && rc == MMF_OK; ++i) rc = step_body(p, X, Y, p->cap_stream);
+  cudaGraph_t graph = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(p->cap_stream, &graph);
+  const long long n = p->launches - before;
+  p->launches = before;   // nothing ran yet: replays are counted when they are enqueued
+  cudaGraphExec_t exec = nullptr;
+  if (rc != MMF_OK || e != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+    cudaGetLastError();
+    if (graph) cudaGraphDestroy(graph);
+    return nullptr;
+  }
+  cudaGraphDestroy(graph);
+  if (p->graphs.size() >= 8) {  // callers that cycle through many field buffers: keep the newest
+    cudaGraphExecDestroy(p->graphs.front().exec);
+    p->graphs.erase(p->graphs.begin());
+  }
+  p->graphs.push_back({X, Y, reps, n, exec});
+  *nlaunch = n;
+  return exec;
+}
+
+// nbody interior steps, from graphs where that pays, else launch by launch
+int run_bodies(mmf_plan* p, cpx* X, cpx* Y, int nbody, cudaStream_t st) {
+  int rc;
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  const bool graphs = !p->timing && nbody >= 2 && p->field_bytes <= kGraphMaxFieldBytes &&
+                      cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs == cudaStreamCaptureStatusNone;
+  if (graphs) {
+    for (const int reps : {kGraphReps, 1}) {
+      if (nbody < reps) continue;
+      long long n = 0;
+      cudaGraphExec_t exec = body_graph(p, X, Y, reps, &n);
+      if (!exec) break;       // capture unavailable: the direct path below takes the rest
+      for (; nbody >= reps; nbody -= reps) {
+        CU(cudaGraphLaunch(exec, st));
+        p->launches += n;
+      }
+    }
+  }
+  for (; nbody > 0; --nbody)
+    if ((rc = step_body(p, X, Y, st)) != MMF_OK) return rc;
+  return MMF_OK;
+}
+
+}  // namespace
+
+// nsteps RK4IP steps; span > 0: after every span-th step the new field is multiplied by `gain` (lumped amplifier)
+static int propagate_impl(mmf_plan* p, void* A_dev, int nsteps, int span, double gain, void* cuda_stream) {
   if (!p || !A_dev || nsteps < 0 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
   if (!p->ws || !on_plan_device(p)) return MMF_EINVAL;
   if (nsteps == 0) return MMF_OK;
+  auto gain_of = [&](int s) { return (span > 0 && (s + 1) % span == 0) ? gain : 1.0; };   // gain applied by step s
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cpx* A = (cpx*)A_dev;
   const bool tiled = p->logn1 > 0;  // N > 4096: every kernel below works in the blocked order (fft_kernels.cuh)
@@ -654,21 +880,42 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
     if (tiled) rc = launch_nlm<NLM_ENTER>(p, A, X, st, Y);               // X <- A, Y <- h N(A) A   (6b bracket)
     else rc = launch_nlm<NLM_PLAIN>(p, X, Y, st);
     if (rc != MMF_OK) return rc;
-    for (int s = 0; s < nsteps; ++s) {
-      if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6a) A_I, (6b) k1
-      if ((rc = launch_nlm<NLM_S23>(p, X, Y, st)) != MMF_OK) return rc;    // (6c), (6d), brackets of 6e/6f
-      if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6e) argument, (6f) first term
-      if (s + 1 < nsteps) rc = launch_nlm<NLM_FINAL_NEXT>(p, X, Y, st);    // (6e)+(6f), next (6b) bracket
-      else if (tiled) rc = launch_nlm<NLM_EXIT>(p, X, Y, st, A);           // (6e)+(6f) into the caller's buffer
-      else rc = launch_nlm<NLM_FINAL>(p, X, Y, st);
-      if (rc != MMF_OK) return rc;
+    for (int s = 0; s < nsteps - 1;) {                                            // all steps but the last
+      int plain = 0;                                                              // steps without an amplifier after them
+      while (s + plain < nsteps - 1 && gain_of(s + plain) == 1.0) ++plain;
+      if ((rc = run_bodies(p, X, Y, plain, st)) != MMF_OK) return rc;
+      s += plain;
+      if (s < nsteps - 1) {
+        if ((rc = step_body(p, X, Y, st, gain_of(s))) != MMF_OK) return rc;     // the last step of a span
+        ++s;
+      }
     }
-    return MMF_OK;
+    const double gl = gain_of(nsteps - 1);
+    if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6a) A_I, (6b) k1
+    if ((rc = launch_nlm<NLM_S23>(p, X, Y, st)) != MMF_OK) return rc;    // (6c), (6d), brackets of 6e/6f
+    if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                      // (6e) argument, (6f) first term
+    if (tiled) rc = launch_nlm<NLM_EXIT>(p, X, Y, st, A, gl);            // (6e)+(6f) into the caller's buffer
+    else rc = launch_nlm<NLM_FINAL>(p, X, Y, st, nullptr, gl);
+    return rc;
   }
   cpx *X = A, *Y = p->Y, *Z = p->Z, *W = p->W;
   if (tiled) {
     if ((rc = to_tiled(p, A, p->V, st)) != MMF_OK) return rc;
     X = p->V;
+  }
+  if (p->general) {
+    // general coupling: one N evaluation per launch, every launch writes a buffer nobody reads in it (nl_general.cuh)
+    if ((rc = launch_nlg<NLG_PLAIN>(p, X, nullptr, nullptr, Y, nullptr, st)) != MMF_OK) return rc;   // Y <- h N(A) A
+    for (int s = 0; s < nsteps; ++s) {
+      if ((rc = apply_D(p, X, Y, 2, st)) != MMF_OK) return rc;                                        // (6a), (6b)
+      if ((rc = launch_nlg<NLG_STAGE2>(p, X, Y, nullptr, Z, nullptr, st)) != MMF_OK) return rc;      // (6c) Z <- k2
+      if ((rc = launch_nlg<NLG_STAGE3>(p, X, Z, Y, W, Y, st)) != MMF_OK) return rc;                  // (6d), brackets
+      if ((rc = apply_D(p, W, Y, 2, st)) != MMF_OK) return rc;                                        // (6e) arg, (6f)
+      if ((rc = launch_nlg<NLG_FINAL>(p, W, nullptr, Y, X, nullptr, st, gain_of(s))) != MMF_OK) return rc;   // (6e) + (6f)
+      if (s + 1 < nsteps && (rc = launch_nlg<NLG_PLAIN>(p, X, nullptr, nullptr, Y, nullptr, st)) != MMF_OK) return rc;
+    }
+    if (tiled && (rc = to_natural(p, X, A, st)) != MMF_OK) return rc;
+    return MMF_OK;
   }
   // the bracket of Eq. (6b) for the first step; later steps get it from NL_FINAL_NEXT
   if ((rc = launch_nl<NL_PLAIN>(p, X, Y, Z, W, st)) != MMF_OK) return rc;
@@ -677,12 +924,22 @@ int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
     if ((rc = launch_nl<NL_STAGE2>(p, X, Y, Z, W, st)) != MMF_OK) return rc;  // (6c) k2
     if ((rc = launch_nl<NL_STAGE3>(p, X, Y, Z, W, st)) != MMF_OK) return rc;  // (6d) k3 and both brackets
     if ((rc = apply_D(p, W, Z, 2, st)) != MMF_OK) return rc;               // (6e) argument, (6f) first term
-    if (s + 1 < nsteps) rc = launch_nl<NL_FINAL_NEXT>(p, X, Y, Z, W, st);  // (6e)+(6f), and next (6b) bracket
-    else rc = launch_nl<NL_FINAL>(p, X, Y, Z, W, st);
+    if (s + 1 < nsteps) rc = launch_nl<NL_FINAL_NEXT>(p, X, Y, Z, W, st, gain_of(s));  // (6e)+(6f), and next (6b) bracket
+    else rc = launch_nl<NL_FINAL>(p, X, Y, Z, W, st, gain_of(s));
     if (rc != MMF_OK) return rc;
   }
   if (tiled && (rc = to_natural(p, X, A, st)) != MMF_OK) return rc;
   return MMF_OK;
+}
+
+int mmf_propagate(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
+  return propagate_impl(p, A_dev, nsteps, 0, 1.0, cuda_stream);
+}
+
+int mmf_propagate_spans(mmf_plan* p, void* A_dev, int nspans, int steps_per_span, double gain, void* cuda_stream) {
+  if (nspans < 0 || steps_per_span < 1 || !std::isfinite(gain)) return MMF_EINVAL;
+  if ((long long)nspans * steps_per_span > 0x7fffffffLL) return MMF_EINVAL;
+  return propagate_impl(p, A_dev, nspans * steps_per_span, steps_per_span, gain, cuda_stream);
 }
 
 int mmf_propagate_ssfm(mmf_plan* p, void* A_dev, int nsteps, void* cuda_stream) {
@@ -735,15 +992,87 @@ int mmf_propagate_ssfm_agrawal(mmf_plan* p, void* A_dev, int nsteps, int niter, 
   return MMF_OK;
 }
 
-int mmf_propagate_host(mmf_plan* p, void* A_host, void* A_dev_scratch, int nsteps, void* cuda_stream) {
-  if (!p || !A_host || !A_dev_scratch || nsteps < 0) return MMF_EINVAL;
+// A stream of host fields through one plan: the copies of field i + 1 (in) and of field i - 1 (out) run on two copy
+// streams while field i propagates, over two device buffers that alternate.  One field alone cannot hide its copies:
+// the first transform needs the whole time axis of every row, the last one produces it.
+int mmf_propagate_host_batch(mmf_plan* p, void* const* A_hosts, int nfields, void* A_dev0, void* A_dev1, int nsteps,
+                             void* cuda_stream) {
+  if (!p || !A_hosts || nfields < 0 || !A_dev0 || nsteps < 0 || !on_plan_device(p)) return MMF_EINVAL;
+  if (nfields > 1 && (!A_dev1 || A_dev1 == A_dev0)) return MMF_EINVAL;
+  for (int i = 0; i < nfields; ++i)
+    if (!A_hosts[i]) return MMF_EINVAL;
+  if (nfields == 0) return MMF_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  CU(cudaMemcpyAsync(A_dev_scratch, A_host, p->field_bytes, cudaMemcpyHostToDevice, st));
-  int rc = mmf_propagate(p, A_dev_scratch, nsteps, cuda_stream);
-  if (rc != MMF_OK) return rc;
-  CU(cudaMemcpyAsync(A_host, A_dev_scratch, p->field_bytes, cudaMemcpyDeviceToHost, st));
-  CU(cudaStreamSynchronize(st));
-  return MMF_OK;
+  void* dev[2] = {A_dev0, A_dev1};
+  if (nfields == 1) {  // nothing to overlap with: everything in order on the caller's stream
+    CU(cudaMemcpyAsync(dev[0], A_hosts[0], p->field_bytes, cudaMemcpyHostToDevice, st));
+    const int rc = mmf_propagate(p, dev[0], nsteps, cuda_stream);
+    if (rc != MMF_OK) return rc;
+    CU(cudaMemcpyAsync(A_hosts[0], dev[0], p->field_bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return MMF_OK;
+  }
+  cudaStream_t sin = nullptr, sout = nullptr;
+  cudaEvent_t ev_start = nullptr, in_done[2] = {nullptr, nullptr}, comp_done[2] = {nullptr, nullptr},
+              out_done[2] = {nullptr, nullptr};
+  int rc = MMF_OK;
+  auto fail = [&](cudaError_t e) { if (e != cudaSuccess && rc == MMF_OK) rc = cuda_fail(e); return e != cudaSuccess; };
+  do {
+    if (fail(cudaStreamCreateWithFlags(&sin, cudaStreamNonBlocking)) ||
+        fail(cudaStreamCreateWithFlags(&sout, cudaStreamNonBlocking)) ||
+        fail(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming)))
+      break;
+    bool bad = false;
+    for (int b = 0; b < 2 && !bad; ++b)
+      bad = fail(cudaEventCreateWithFlags(&in_done[b], cudaEventDisableTiming)) ||
+            fail(cudaEventCreateWithFlags(&comp_done[b], cudaEventDisableTiming)) ||
+            fail(cudaEventCreateWithFlags(&out_done[b], cudaEventDisableTiming));
+    if (bad) break;
+    // the copy streams start after the work already enqueued on the caller's stream
+    if (fail(cudaEventRecord(ev_start, st)) || fail(cudaStreamWaitEvent(sin, ev_start, 0)) ||
+        fail(cudaStreamWaitEvent(sout, ev_start, 0)))
+      break;
+    auto copy_in = [&](int i) {
+      const int b = i & 1;
+      if (i >= 2 && fail(cudaStreamWaitEvent(sin, out_done[b], 0))) return;   // field i - 2 has left this buffer
+      if (fail(cudaMemcpyAsync(dev[b], A_hosts[i], p->field_bytes, cudaMemcpyHostToDevice, sin))) return;
+      fail(cudaEventRecord(in_done[b], sin));
+    };
+    copy_in(0);
+    for (int i = 0; i < nfields && rc == MMF_OK; ++i) {
+      const int b = i & 1;
+      if (i + 1 < nfields) copy_in(i + 1);
+      if (rc != MMF_OK || fail(cudaStreamWaitEvent(st, in_done[b], 0))) break;
+      if ((rc = mmf_propagate(p, dev[b], nsteps, cuda_stream)) != MMF_OK) break;
+      if (fail(cudaEventRecord(comp_done[b], st)) || fail(cudaStreamWaitEvent(sout, comp_done[b], 0)) ||
+          fail(cudaMemcpyAsync(A_hosts[i], dev[b], p->field_bytes, cudaMemcpyDeviceToHost, sout)) ||
+          fail(cudaEventRecord(out_done[b], sout)))
+        break;
+    }
+    // the call returns with every field back on the host; the caller's stream is ordered after the last copy out
+    if (sout) fail(cudaStreamSynchronize(sout));
+    if (sin) fail(cudaStreamSynchronize(sin));
+    fail(cudaStreamSynchronize(st));
+  } while (0);
+  if (rc != MMF_OK) {  // drain whatever was enqueued before the failure
+    if (sin) cudaStreamSynchronize(sin);
+    if (sout) cudaStreamSynchronize(sout);
+    cudaStreamSynchronize(st);
+  }
+  for (int b = 0; b < 2; ++b) {
+    if (in_done[b]) cudaEventDestroy(in_done[b]);
+    if (comp_done[b]) cudaEventDestroy(comp_done[b]);
+    if (out_done[b]) cudaEventDestroy(out_done[b]);
+  }
+  if (ev_start) cudaEventDestroy(ev_start);
+  if (sin) cudaStreamDestroy(sin);
+  if (sout) cudaStreamDestroy(sout);
+  return rc;
+}
+
+int mmf_propagate_host(mmf_plan* p, void* A_host, void* A_dev_scratch, int nsteps, void* cuda_stream) {
+  void* one[1] = {A_host};
+  return mmf_propagate_host_batch(p, A_host ? one : nullptr, 1, A_dev_scratch, nullptr, nsteps, cuda_stream);
 }
 
 int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
@@ -759,6 +1088,15 @@ int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
 
 int mmf_apply_nonlinear(mmf_plan* p, const void* U_dev, void* OUT_dev, void* cuda_stream) {
   if (!p || !U_dev || !OUT_dev || (((size_t)U_dev | (size_t)OUT_dev) & 15) != 0 || !on_plan_device(p)) return MMF_EINVAL;
+  if (p->general) {
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (U_dev != OUT_dev) return launch_nlg<NLG_PLAIN>(p, (const cpx*)U_dev, nullptr, nullptr, (cpx*)OUT_dev, nullptr, st);
+    if (!p->ws) return MMF_EINVAL;   // in place: through the workspace (a CTA reads rows its partner writes)
+    int rc = launch_nlg<NLG_PLAIN>(p, (const cpx*)U_dev, nullptr, nullptr, p->Y, nullptr, st);
+    if (rc != MMF_OK) return rc;
+    CU(cudaMemcpyAsync(OUT_dev, p->Y, p->field_bytes, cudaMemcpyDeviceToDevice, st));
+    return MMF_OK;
+  }
   if (p->nlm_nk > 0) return launch_nlm<NLM_PLAIN>(p, (const cpx*)U_dev, (cpx*)OUT_dev, (cudaStream_t)cuda_stream);
   return launch_nl<NL_PLAIN>(p, (cpx*)U_dev, (cpx*)OUT_dev, nullptr, nullptr, (cudaStream_t)cuda_stream);
 }

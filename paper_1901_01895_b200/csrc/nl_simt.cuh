@@ -22,6 +22,7 @@ struct NlParams {
   cpx* W;
   const double* __restrict__ kappa;  // [M][M]
   double hg;
+  double gain;  // NL_FINAL / NL_FINAL_NEXT: amplitude factor of a lumped amplifier applied to the new field (1 = none)
   int M;
   long long N;
 };
@@ -89,7 +90,7 @@ __global__ void __launch_bounds__(MMF_NL_T* MMF_NL_WARPS) k_nl(NlParams p) {
         } else {
           const cpx z = p.Z[i];
           const double sixth = 1.0 / 6.0;
-          const cpx an = make_double2(fma(sixth, k.x, z.x), fma(sixth, k.y, z.y));
+          const cpx an = make_double2(p.gain * fma(sixth, k.x, z.x), p.gain * fma(sixth, k.y, z.y));
           p.X[i] = an;
           pw2 += an.x * an.x + an.y * an.y;
         }

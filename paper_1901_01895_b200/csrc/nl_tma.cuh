@@ -7,7 +7,8 @@
 //               X <- X + k3  (the argument of Eq. 6e),  Y <- X + Y/6 + k2/3 + k3/3  (the bracket of Eq. 6f), IN PLACE.
 //               Eq. (6c) and (6d) have no transform between them, so both are evaluated in one pass: 4 F of traffic
 //               instead of the 8 F two kernels need.
-//   NLM_FINAL   X = u4, Y = exp(h/2 L)[...]:  X <- Y + NL(X)/6                   (Eq. 6e + 6f; Y untouched)
+//   NLM_FINAL   X = u4, Y = exp(h/2 L)[...]:  X <- gain (Y + NL(X)/6)            (Eq. 6e + 6f; Y untouched; gain = 1
+//               except at the end of a fibre span, where it is the lumped amplifier of PAPER.md:255)
 //   NLM_FINAL_NEXT  as NLM_FINAL, then Y <- NL(X_new)                           (the next step's Eq. 6b bracket)
 //   NLM_ENTER   first kernel of a propagation in the blocked order (fft_kernels.cuh): reads tile tn(t) of the caller's
 //               field A (NATURAL order) and writes tile t of X <- A and of Y <- NL(A) (blocked order): the layout
@@ -52,6 +53,7 @@ enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3, NLM_RK4 = 
 struct NltParams {
   const double* __restrict__ kappa;  // [M][M] row-major
   double hg;
+  double gain;       // FINAL / FINAL_NEXT / EXIT: amplitude factor of a lumped amplifier applied to the new field (1 = none)
   int M;
   int NW;            // compute warps = ceil(M / 8); the producer is warp NW
   int logn1, logn2, logwb;  // NLM_ENTER / NLM_EXIT: geometry of the blocked order (N = N1 N2, WB columns per block)
@@ -318,7 +320,10 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
 #pragma unroll
         for (int pol = 0; pol < 2; ++pol)
 #pragma unroll
-          for (int i = 0; i < 2; ++i) sx[e0 + pol * MMF_NLM_T + i] = axpy(sixth, times_ig(u[pol][i], g1[i]), y[pol][i]);
+          for (int i = 0; i < 2; ++i) {
+            const cpx an = axpy(sixth, times_ig(u[pol][i], g1[i]), y[pol][i]);
+            sx[e0 + pol * MMF_NLM_T + i] = make_double2(p.gain * an.x, p.gain * an.y);
+          }
       }
     } else {
       // ---- round 2 -------------------------------------------------------------------------------------------
@@ -328,7 +333,12 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
           const cpx k = times_ig(u[pol][i], g1[i]);  // k2 resp. k4
-          v[pol][i] = (MODE == NLM_S23) ? axpy(0.5, k, x[pol][i]) : axpy(sixth, k, y[pol][i]);
+          if constexpr (MODE == NLM_S23) {
+            v[pol][i] = axpy(0.5, k, x[pol][i]);
+          } else {
+            const cpx an = axpy(sixth, k, y[pol][i]);
+            v[pol][i] = make_double2(p.gain * an.x, p.gain * an.y);   // the lumped amplifier acts before the next N
+          }
         }
       if (valid)
         *reinterpret_cast<double2*>(Pb1 + a * MMF_NLM_PSTRIDE + 2 * q) =

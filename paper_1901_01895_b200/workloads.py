@@ -60,6 +60,15 @@ class Problem:
         self.kappa = np.ascontiguousarray(kap + kap.T + np.eye(self.M))
         self._c = c
 
+    def kappa_general(self, seed=0):
+        """A [2M][2M] per-polarisation coupling matrix for this config: the config's mode-pair
+        strengths kappa_ab, same-polarisation coupling 1 and cross-polarisation 2/3 (the ratio of a linearly
+        birefringent fibre), and a seeded +-10 % spread per entry, so the matrix is NOT symmetric."""
+        rng = np.random.default_rng([SEED_BASE, self.cfg, 7, int(seed)])
+        pol = np.array([[1.0, 2.0 / 3.0], [2.0 / 3.0, 1.0]])
+        k2 = np.kron(self.kappa, pol)
+        return np.ascontiguousarray(k2 * rng.uniform(0.9, 1.1, size=k2.shape))
+
     # ---- input waveforms -------------------------------------------------------------------------------
     def row(self, r):
         """Input samples of field r = 2a+p (complex128, length N), seeded per row."""

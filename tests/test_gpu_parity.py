@@ -259,3 +259,63 @@ def test_propagate_non_symmetric_kappa_no_loss_single_sample_tile(mmf, torch, or
     want = orc.rk4ip(A, dt, h, 0.0, beta, 0.1, kappa, steps)
     assert workloads.rel_l2_per_field(want, A).min() > 1e-3
     assert workloads.rel_l2_per_field(X.cpu().numpy(), want).max() <= TOL_FIELD
+
+
+# ------------------------------------------------------------------------ spans with lumped amplifiers
+@pytest.mark.parametrize("cfg,M,logn,nspans,k,general", [(0, 2, 12, 3, 4, False), (1, 6, 14, 2, 3, False),
+                                                          (3, 120, 13, 2, 2, False), (3, 122, 13, 2, 2, False),
+                                                          (2, 5, 13, 2, 3, True), (1, 3, 16, 1, 40, False)])
+def test_spans_match_oracle(mmf, torch, orc, cfg, M, logn, nspans, k, general):
+    """mmf_propagate_spans: the amplifier gain rides on the last kernel of every span (graph-replayed bodies in
+    between for the small cases); against the oracle's rk4ip_spans."""
+    import math
+    p = workloads.problem(cfg, M=M, N=1 << logn)
+    A = p.field() * 2.0
+    kap = p.kappa_general() if general else p.kappa
+    gain = math.exp(p.alpha * p.h * k / 2) * 1.7          # more than the loss: the nonlinearity grows span by span
+    pl = mmf.Plan(p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, general=general)
+    X = to_dev(torch, A)
+    pl.propagate_spans(X, nspans, k, gain)
+    want = orc.rk4ip_spans(A, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, nspans, k, gain, general=general)
+    err = workloads.rel_l2_per_field(X.cpu().numpy(), want)
+    assert err.max() <= TOL_FIELD, (err.max(), err.argmax())
+    nogain = orc.rk4ip_spans(A, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, nspans, k, 1.0, general=general)
+    assert workloads.rel_l2_per_field(want, nogain).min() > 0.1
+
+
+def test_graph_replay_is_bit_identical_to_direct_launches(mmf, torch):
+    """small problems replay their step body from a CUDA graph; with per-launch timing on they launch directly:
+    both must give the same bits, for step counts that mix 16-step graphs, 1-step graphs and the direct tail."""
+    p = workloads.problem(0, N=1 << 12)
+    A = p.field()
+    pl = plan_for(mmf, p)
+    for steps in (1, 2, 3, 18, 37):
+        X = to_dev(torch, A)
+        n0 = pl.launch_count()
+        pl.propagate(X, steps)
+        n_graph = pl.launch_count() - n0
+        Y = to_dev(torch, A)
+        pl.set_timing(True)
+        n0 = pl.launch_count()
+        pl.propagate(Y, steps)
+        n_direct = pl.launch_count() - n0
+        pl.set_timing(False)
+        assert np.array_equal(X.cpu().numpy(), Y.cpu().numpy()), steps
+        assert n_graph == n_direct == 1 + 4 * steps
+
+
+def test_propagate_host_batch(mmf, torch, orc):
+    """five host fields (a launch-power sweep) through two device buffers with overlapped copies; every field must
+    come back as the oracle propagates it."""
+    p = workloads.problem(1, M=3, N=1 << 14, steps=4)
+    A = p.field()
+    scales = [0.5, 1.0, 1.5, 2.0, 2.5]
+    hosts = [torch.from_numpy(A * s).pin_memory() for s in scales]
+    pl = plan_for(mmf, p)
+    d0 = torch.empty((2 * p.M, p.N), dtype=torch.complex128, device="cuda:0")
+    d1 = torch.empty_like(d0)
+    pl.propagate_host_batch(hosts, d0, d1, 4)
+    for H, s in zip(hosts, scales):
+        want = orc.rk4ip(A * s, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, 4)
+        assert workloads.rel_l2_per_field(H.numpy(), want).max() <= TOL_FIELD
+    pl.propagate_host_batch(hosts[:1], d0, None, 0)                       # one field, zero steps: a round trip

@@ -96,3 +96,44 @@ def test_general_fourth_order_against_independent_solution_of_eq1(orc):
 def test_packed_size_the_paper_prints():
     M = 120
     assert (2 * M * 2 * M) // 2 + M == 28920                  # PAPER.md:176 "(2M 2M)/2 + M", :182 "28920"
+
+
+# ------------------------------------------------------------------------------- spans with lumped amplifiers
+def test_spans_gamma_zero_loss_is_compensated_exactly(orc):
+    """gamma = 0, gain = exp(alpha L_span / 2): after every span the spectrum has its input magnitude back and the
+    field is the lossless linear solution over the whole link (closed form written with numpy)."""
+    M, N, dt, h, k, nsp = 2, 64, 0.7, 3.0, 4, 3
+    rng = np.random.default_rng(14)
+    X = rand_c(rng, 2 * M, N)
+    X[:, N // 2] = 0
+    A = np.fft.ifft(X, axis=1)
+    alpha = 0.05
+    beta = np.array([[0.01, 0.03, -0.05, 0.004], [-0.02, -0.01, -0.03, 0.002]])
+    w = 2 * np.pi * np.fft.fftfreq(N, d=dt)
+    want = np.empty_like(A)
+    for r in range(2 * M):
+        L = np.zeros(N, dtype=complex)
+        for n, b in enumerate(beta[r // 2]):
+            L = L + 1j * (1j ** n) / math.factorial(n) * b * (1j * w) ** n
+        want[r] = np.fft.ifft(np.exp(L * h * k * nsp) * np.fft.fft(A[r]))        # alpha = 0 over the whole link
+    got = orc.rk4ip_spans(A, dt, h, alpha, beta, 0.0, np.eye(M), nsp, k, math.exp(alpha * h * k / 2), nthreads=1)
+    assert rel(got, want) <= 1e-13
+    assert abs(np.sum(np.abs(got) ** 2) / np.sum(np.abs(A) ** 2) - 1.0) <= 1e-13
+
+
+def test_spans_amplifier_acts_between_spans_not_inside(orc):
+    """with nonlinearity the place of the gain matters: gain after each span differs from one gain at the end (same
+    total gain) and from no gain — and equals propagating span by span with the amplitude scaled in between."""
+    M, N, dt, h, k = 2, 32, 1.0, 2.0, 3
+    rng = np.random.default_rng(15)
+    A = rand_c(rng, 2 * M, N) * 0.6
+    beta = np.array([[0.0, 0.01, -0.02, 0.001], [0.0, -0.01, -0.03, 0.001]])
+    kappa = np.array([[1.0, 0.4], [0.7, 1.0]])
+    alpha, gamma, g = 0.05, 0.05, 1.3
+    got = orc.rk4ip_spans(A, dt, h, alpha, beta, gamma, kappa, 2, k, g, nthreads=1)
+    by_hand = orc.rk4ip(orc.rk4ip(A, dt, h, alpha, beta, gamma, kappa, k, nthreads=1) * g, dt, h, alpha, beta, gamma,
+                        kappa, k, nthreads=1) * g
+    assert np.array_equal(got, by_hand)
+    end_only = orc.rk4ip(A, dt, h, alpha, beta, gamma, kappa, 2 * k, nthreads=1) * g * g
+    assert rel(got, end_only) > 1e-3
+    assert np.array_equal(orc.rk4ip_spans(A, dt, h, alpha, beta, gamma, kappa, 0, k, g), A)
