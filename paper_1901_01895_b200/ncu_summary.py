@@ -28,10 +28,12 @@ METRICS = {
     "ms": ("gpu__time_duration.sum", 1e-6),                      # ns -> ms
     "dram_read_bytes": ("dram__bytes_read.sum", None),
     "dram_write_bytes": ("dram__bytes_write.sum", None),
-    "dram_pct": ("dram__throughput.avg.pct_of_peak_sustained_elapsed", 1.0),
+    "dram_pct": ("gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", 1.0),
     "fp64_pipe_pct": ("sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active", 1.0),
     "lsu_data_pipe_pct": ("l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed", 1.0),
-    "issue_pct": ("sm__issue_active.avg.pct_of_peak_sustained_active", 1.0),
+    "issue_pct": ("sm__inst_issued.avg.pct_of_peak_sustained_active", 1.0),
+    "smem_wavefronts": ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", 1.0),
+    "smem_bank_conflicts": ("l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum", 1.0),
     "registers": ("launch__registers_per_thread", 1.0),
     "warp_inst": ("smsp__inst_executed.sum", 1.0),
     "dadd": ("smsp__sass_thread_inst_executed_op_dadd_pred_on.sum", 1.0),
