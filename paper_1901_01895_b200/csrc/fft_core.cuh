@@ -235,7 +235,10 @@ __device__ __forceinline__ void stage_math(cpx (&v)[16], int base, const cpx* __
 // FENCE: also synchronise after the last exchange read (needed when the caller's next use of the buffer does not
 // start with the slots this thread read last, i.e. when the chain is not followed by its adjoint).
 // PRESYNC: also synchronise before the FIRST exchange write (needed when the caller took v from the exchange buffer
-// itself in a different layout — a tile staged there by TMA — so that nobody overwrites a value not yet read).
+// itself UNSWIZZLED — a tile staged there by TMA — so that nobody overwrites a value not yet read).  A WARP barrier is
+// enough: thread t then read the slots base | j << LO and writes swz(base | j << LO), and the swizzle changes bits
+// [2:0] of a slot only — lane or register bits, never warp bits — so the slots a thread overwrites were read by
+// lanes of its own warp.
 template <int LOGTOT, int LOGP, int LOGW, int REMAIN, int NST, int SIGN, bool FENCE, bool PRESYNC = false>
 __device__ __forceinline__ void fft_dif(cpx (&v)[16], cpx* __restrict__ s, int t, const cpx* __restrict__ tab, int bar) {
   constexpr int LR = stage_lr(REMAIN, NST), LOGM = REMAIN - LR, LO = stage_lo(LOGM, LOGW, LOGTOT);
@@ -243,7 +246,7 @@ __device__ __forceinline__ void fft_dif(cpx (&v)[16], cpx* __restrict__ s, int t
   stage_math<LOGTOT, LOGW, LOGM, LR, SIGN, true>(v, base, tab + tw_offset(LOGP, REMAIN, NST));
   if constexpr (NST > 1) {
     constexpr int LR2 = stage_lr(LOGM, NST - 1), LO2 = stage_lo(LOGM - LR2, LOGW, LOGTOT);
-    if constexpr (PRESYNC && REMAIN == LOGP) group_barrier(bar, MMF_GROUP_THREADS);
+    if constexpr (PRESYNC && REMAIN == LOGP) __syncwarp();
     tile_sts<LO>(v, s, base);
     exchange_barrier<LO, LO2>(bar);
     tile_lds<LO2>(v, s, stage_base<LO2>(t));
@@ -261,7 +264,7 @@ __device__ __forceinline__ void fft_dit(cpx (&v)[16], cpx* __restrict__ s, int t
   if constexpr (NST > 1) {
     constexpr int LR2 = stage_lr(LOGM, NST - 1), LO2 = stage_lo(LOGM - LR2, LOGW, LOGTOT);
     fft_dit<LOGTOT, LOGP, LOGW, LOGM, NST - 1, SIGN, false, PRESYNC>(v, s, t, tab, bar);
-    if constexpr (PRESYNC && NST == 2) group_barrier(bar, MMF_GROUP_THREADS);
+    if constexpr (PRESYNC && NST == 2) __syncwarp();
     tile_sts<LO2>(v, s, stage_base<LO2>(t));
     exchange_barrier<LO2, LO>(bar);
     tile_lds<LO>(v, s, base);

@@ -19,6 +19,7 @@
 #pragma once
 #include "async_copy.cuh"
 #include "fft_core.cuh"
+#include "tmem_exchange.cuh"
 
 namespace mmf {
 
@@ -220,7 +221,7 @@ k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
       }
       fft_dif<MMF_TILE_LOG, LOGN1, LOGW, LOGN1, NST, +1, false, true>(v, s, t, tab, bar);
       apply_interpass<false>(v, ip[t], ip[256 + c], ip[256 + W + c]);
-      group_barrier(bar, MMF_GROUP_THREADS);  // everybody has read the last exchange
+      __syncwarp();  // the unswizzled slots written next were read, swizzled, by lanes of this warp (fft_core.cuh, PRESYNC)
       tile_sts_linear<LOL>(v, s, basel);
     } else {
       tile_lds_linear<LOL>(v, s, basel);
@@ -231,7 +232,7 @@ k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
       }
       apply_interpass<true>(v, t0, sA, sB);
       fft_dit<MMF_TILE_LOG, LOGN1, LOGW, LOGN1, NST, -1, false, true>(v, s, t, tab, bar);
-      group_barrier(bar, MMF_GROUP_THREADS);
+      __syncwarp();
       tile_sts_linear<LO1>(v, s, base1);
     }
     // hand the finished tile to the async proxy: every thread's writes are fenced, the first thread stores
@@ -361,7 +362,11 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
   // global memory and parks them in tensor memory (64 columns of the thread's own lane), the others read them back
   // from there — no global-load latency, no LSU traffic, no shared memory (none is left).
   constexpr bool ECACHE = MODE == 0 && !SINGLE;
-  constexpr uint32_t TMEM_COLS = 256;  // 4 warps share a lane quarter: 4 x 64 columns
+  // 4096-point transforms: the exchange between the last two stages goes through tensor memory (tmem_exchange.cuh),
+  // 64 more columns per warp
+  constexpr bool TMX = LOGN2 == 12;
+  constexpr uint32_t WARP_COLS = TMX ? 128 : 64;
+  constexpr uint32_t TMEM_COLS = 4 * WARP_COLS;  // 4 warps share a lane quarter
   uint32_t* tmem_word = reinterpret_cast<uint32_t*>(done + G);
   if (threadIdx.x == 0) {
 #pragma unroll
@@ -370,7 +375,7 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
     for (int i = 0; i < G; ++i) mbar_init(&done[i], MMF_GROUP_THREADS);
     mbar_init_fence();
   }
-  if constexpr (ECACHE) {
+  if constexpr (ECACHE || TMX) {
     if (threadIdx.x < 32) {
       __syncwarp();  // reconverge after the single-thread block above: tcgen05.alloc is .sync.aligned
       tmem_alloc(tmem_word, TMEM_COLS);
@@ -378,19 +383,21 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
     tmem_fence_before_sync();
   }
   load_stage_tables<TWN>(tab, p.twtab);  // ends with __syncthreads
-  uint32_t taddr = 0;
-  if constexpr (ECACHE) {
+  uint32_t taddr = 0;   // this warp's columns: [0, 64) the E values of the item, [64, 128) the exchange buffer (TMX)
+  if constexpr (ECACHE || TMX) {
     tmem_fence_after_sync();
     const uint32_t warp = threadIdx.x >> 5;
-    taddr = *tmem_word + (((warp & 3) * 32) << 16) + (warp >> 2) * 64;
+    taddr = *tmem_word + (((warp & 3) * 32) << 16) + (warp >> 2) * WARP_COLS;
   }
   int cached_item = -1;
   const int grp = threadIdx.x / MMF_GROUP_THREADS, t = threadIdx.x % MMF_GROUP_THREADS;
   const bool elect = t == 0;
   const int bar = 1 + grp;
   const int base1 = stage_base<LO1>(t);
-  const int cht = (t << 4) >> LOGN2;                 // chunk (inside the tile) of this thread's last-stage values
-  const int tq = t & ((1 << (LOGN2 - 4)) - 1);
+  const Tm12 lay = tm12_layout(t);
+  const int tl = TMX ? lay.tv : t;                   // slot >> 4 of this thread's last-stage values
+  const int cht = (tl << 4) >> LOGN2;                // their chunk (inside the tile)
+  const int tq = tl & ((1 << (LOGN2 - 4)) - 1);
   const int logn1 = p.logn1;
   const int logsub = (SINGLE ? 0 : 1) + (p.nbuf > 1 ? 1 : 0);   // sub-tiles per item: nbuf (SINGLE) or 2 nbuf
   const long long items = SINGLE ? ((p.nchunks + (1 << LOGB) - 1) >> LOGB) : ((long long)p.M << (logn1 - LOGB));
@@ -480,6 +487,28 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
     const bool refill = elect && tt >= G && tt - G + S < ntile_i;
     const int b = tt % S;
     cpx* s = ring + ((size_t)b << MMF_TILE_LOG);
+    if constexpr (ECACHE) {
+      // First tile of an item: fetch the thread's 16 E values into tensor memory NOW, while no tile is held in
+      // registers — all 16 loads in flight at once (one latency per item instead of one per pair of values), and
+      // every sub-tile of the item reads them back from there.
+      long long chunk0, item;
+      int buf;
+      tile_geom(tt, chunk0, buf, item);
+      if ((int)item != cached_item) {  // uniform over the group
+        const long long a = item >> (logn1 - LOGB), tau = item & ((1LL << (logn1 - LOGB)) - 1);
+        const cpx* e = p.E + (((a << logn1) + (tau << LOGB) + cht) << LOGN2) + tq;
+        cpx ev[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) ev[j] = __ldg(e + (j << (LOGN2 - 4)));
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          const cpx pr[2] = {ev[2 * c], ev[2 * c + 1]};
+          tmem_st_c2(taddr + 8 * c, pr);
+        }
+        tmem_wait_st();
+        cached_item = (int)item;
+      }
+    }
     mbar_wait(&full[b], (uint32_t)((tt / S) & 1));
     cpx v[16];
     tile_lds_linear<LO1>(v, s, base1);
@@ -487,51 +516,40 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
       tma_store_wait_read();
       issue_load(tt - G + S);
     }
-    fft_dif<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, +1, MODE == 1, true>(v, s, t, tab, bar);
+    if constexpr (TMX) fft12_dif_tm<+1>(v, s, lay, tab, bar, taddr + 64);
+    else fft_dif<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, +1, MODE == 1, true>(v, s, t, tab, bar);
     if constexpr (MODE == 0) {
-      {
+      if constexpr (ECACHE) {   // the item's E values are in tensor memory (loaded at the top of the item's first tile)
+#pragma unroll
+        for (int hb = 0; hb < 2; ++hb) {   // two batches of eight: two tensor-memory latencies per tile
+          int wa[4][8];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) tmem_ld_issue8(wa[c], taddr + 32 * hb + 8 * c);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) tmem_ld_wait8(wa[c]);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            cpx ev[2];
+            tmem_words_to_c2(ev, wa[c]);
+            v[8 * hb + 2 * c] = cmul(v[8 * hb + 2 * c], ev[0]);
+            v[8 * hb + 2 * c + 1] = cmul(v[8 * hb + 2 * c + 1], ev[1]);
+          }
+        }
+      } else {
         long long chunk0, item;
         int buf;
         tile_geom(tt, chunk0, buf, item);
-        if (!SINGLE || chunk0 + cht < p.nchunks) {
-          long long ech;  // table chunk of this thread's last-stage values
-          if constexpr (SINGLE) {
-            ech = (chunk0 + cht) >> 1;  // chunk = row, table chunk = mode
-          } else {
-            const long long a = item >> (logn1 - LOGB), tau = item & ((1LL << (logn1 - LOGB)) - 1);
-            ech = (a << logn1) + (tau << LOGB) + cht;
-          }
-          const cpx* e = p.E + (ech << LOGN2) + tq;
-          if constexpr (ECACHE) {
-            if ((int)item == cached_item) {  // uniform over the group
+        if (chunk0 + cht < p.nchunks) {
+          const cpx* e = p.E + (((chunk0 + cht) >> 1) << LOGN2) + tq;  // chunk = row, table chunk = mode
 #pragma unroll
-              for (int c = 0; c < 8; ++c) {
-                cpx ev[2];
-                tmem_ld_c2(ev, taddr + 8 * c);
-                v[2 * c] = cmul(v[2 * c], ev[0]);
-                v[2 * c + 1] = cmul(v[2 * c + 1], ev[1]);
-              }
-            } else {
-#pragma unroll
-              for (int c = 0; c < 8; ++c) {
-                cpx ev[2];
-                ev[0] = __ldg(e + ((2 * c) << (LOGN2 - 4)));
-                ev[1] = __ldg(e + ((2 * c + 1) << (LOGN2 - 4)));
-                tmem_st_c2(taddr + 8 * c, ev);
-                v[2 * c] = cmul(v[2 * c], ev[0]);
-                v[2 * c + 1] = cmul(v[2 * c + 1], ev[1]);
-              }
-              tmem_wait_st();
-              cached_item = (int)item;
-            }
-          } else {
-#pragma unroll
-            for (int j = 0; j < 16; ++j) v[j] = cmul(v[j], __ldg(e + (j << (LOGN2 - 4))));
-          }
+          for (int j = 0; j < 16; ++j) v[j] = cmul(v[j], __ldg(e + (j << (LOGN2 - 4))));
         }
       }
-      fft_dit<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, -1, false>(v, s, t, tab, bar);
-      group_barrier(bar, MMF_GROUP_THREADS);  // everybody has read the last exchange
+      if constexpr (TMX) fft12_dit_tm<-1>(v, s, lay, tab, bar, taddr + 64);
+      else fft_dit<MMF_TILE_LOG, LOGN2, 0, LOGN2, NST, -1, false>(v, s, t, tab, bar);
+      // the unswizzled slots written next were read, in the last exchange, swizzled by lanes of the same warp (the
+      // swizzles touch bits [2:0] of a slot only): a warp barrier orders the two
+      __syncwarp();
       tile_sts_linear<LO1>(v, s, base1);
       fence_proxy_async_smem();
       mbar_arrive(&done[grp]);
@@ -555,13 +573,13 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
       if (!SINGLE || chunk0 + cht < p.nchunks) {
         cpx* g = p.OUT + (chunk0 << LOGN2);
 #pragma unroll
-        for (int j = 0; j < 16; ++j) g[(t << 4) + j] = v[j];
+        for (int j = 0; j < 16; ++j) g[(tl << 4) + j] = v[j];
       }
       group_barrier(bar, MMF_GROUP_THREADS);  // the slot may be refilled
     }
   }
   if (elect) tma_store_wait_all();
-  if constexpr (ECACHE) {
+  if constexpr (ECACHE || TMX) {
     tmem_fence_before_sync();
     __syncthreads();
     if (threadIdx.x < 32) tmem_dealloc(*tmem_word, TMEM_COLS);

@@ -334,10 +334,12 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
 template <int DIR>
 int launch_cols(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   switch (p->logn1) {
+#ifndef MMF_LEAN_BUILD   // MMF_LEAN_BUILD: config-4 instantiations only (quick builds for kernel experiments)
     case 6: return launch_cols_t<6, DIR>(p, X0, X1, nbuf, st);
     case 8: return launch_cols_t<8, DIR>(p, X0, X1, nbuf, st);
-    case 10: return launch_cols_t<10, DIR>(p, X0, X1, nbuf, st);
     case 12: return launch_cols_t<12, DIR>(p, X0, X1, nbuf, st);
+#endif
+    case 10: return launch_cols_t<10, DIR>(p, X0, X1, nbuf, st);
     default: return MMF_EINVAL;
   }
 }
@@ -376,15 +378,20 @@ int launch_rows(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cpx* OUT, cudaStream_t 
   if (p->logn1 == 0) {
     switch (p->logn2) {
 #define MMF_ROWS_CASE(L) case L: return launch_rows_t<L, MODE, true>(p, X0, X1, nbuf, OUT, st);
+#ifndef MMF_LEAN_BUILD
       MMF_ROWS_CASE(4) MMF_ROWS_CASE(5) MMF_ROWS_CASE(6) MMF_ROWS_CASE(7) MMF_ROWS_CASE(8) MMF_ROWS_CASE(9)
-      MMF_ROWS_CASE(10) MMF_ROWS_CASE(11) MMF_ROWS_CASE(12)
+      MMF_ROWS_CASE(10) MMF_ROWS_CASE(11)
+#endif
+      MMF_ROWS_CASE(12)
 #undef MMF_ROWS_CASE
       default: return MMF_EINVAL;
     }
   }
   switch (p->logn2) {
 #define MMF_ROWS_CASE(L) case L: return launch_rows_t<L, MODE, false>(p, X0, X1, nbuf, OUT, st);
+#ifndef MMF_LEAN_BUILD
     MMF_ROWS_CASE(6) MMF_ROWS_CASE(7) MMF_ROWS_CASE(8) MMF_ROWS_CASE(9) MMF_ROWS_CASE(10) MMF_ROWS_CASE(11)
+#endif
     MMF_ROWS_CASE(12)
 #undef MMF_ROWS_CASE
     default: return MMF_EINVAL;
@@ -544,9 +551,12 @@ template <int MODE>
 int launch_nlm(mmf_plan* p, const cpx* A, cpx* B, cudaStream_t st, cpx* C = nullptr, double gain = 1.0) {
   switch (p->nlm_nk) {
 #define MMF_NLM_CASE(NKV) case NKV: return launch_nlm_t<NKV, MODE>(p, A, B, C, st, gain);
-    MMF_NLM_CASE(1) MMF_NLM_CASE(2) MMF_NLM_CASE(3) MMF_NLM_CASE(4) MMF_NLM_CASE(6) MMF_NLM_CASE(8) MMF_NLM_CASE(9)
-    MMF_NLM_CASE(12) MMF_NLM_CASE(16) MMF_NLM_CASE(20) MMF_NLM_CASE(24) MMF_NLM_CASE(28) MMF_NLM_CASE(30)
+#ifndef MMF_LEAN_BUILD
+    MMF_NLM_CASE(2) MMF_NLM_CASE(3) MMF_NLM_CASE(4) MMF_NLM_CASE(6) MMF_NLM_CASE(8) MMF_NLM_CASE(9)
+    MMF_NLM_CASE(12) MMF_NLM_CASE(16) MMF_NLM_CASE(20) MMF_NLM_CASE(24) MMF_NLM_CASE(28)
     MMF_NLM_CASE(32)
+#endif
+    MMF_NLM_CASE(1) MMF_NLM_CASE(30)
 #undef MMF_NLM_CASE
     default: return MMF_EINVAL;
   }
