@@ -37,11 +37,19 @@ __host__ __device__ inline int slot_to_bin_rt(int logn, int p) {
   return k;
 }
 
-// copy the stage tables of a transform into shared memory (whole CTA), then synchronise
+// The stage tables of a transform travel to shared memory as ONE bulk copy issued by the CTA's first thread right after
+// the barrier initialisation (no thread-level loads, and the copy overlaps the rest of the prologue and the first
+// tile loads); every thread waits on its mbarrier once, before the first table read.
 template <int ENTRIES>
-__device__ __forceinline__ void load_stage_tables(cpx* __restrict__ tab, const cpx* __restrict__ src) {
-  for (int i = threadIdx.x; i < ENTRIES; i += blockDim.x) tab[i] = src[i];
-  __syncthreads();
+__device__ __forceinline__ void request_stage_tables(cpx* __restrict__ tab, const cpx* __restrict__ src, uint64_t* tabbar) {
+  if constexpr (ENTRIES > 0) {
+    mbar_arrive_expect_tx(tabbar, ENTRIES * (int)sizeof(cpx));
+    bulk_load_1d(tab, src, ENTRIES * (int)sizeof(cpx), tabbar);
+  }
+}
+template <int ENTRIES>
+__device__ __forceinline__ void await_stage_tables(uint64_t* tabbar) {
+  if constexpr (ENTRIES > 0) mbar_wait(tabbar, 0);
 }
 
 // ---------------------------------------------------------------------------------------------------- pass A / C
@@ -144,16 +152,21 @@ k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
   cpx* tab = ipts + S * IPT;
   uint64_t* full = reinterpret_cast<uint64_t*>(tab + ((TWN + 7) & ~7));
   uint64_t* done = full + S;
+  uint64_t* tabbar = done + G;
+  pdl_launch_dependents();
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
 #pragma unroll
     for (int i = 0; i < G; ++i) mbar_init(&done[i], MMF_GROUP_THREADS);
+    mbar_init(tabbar, 1);
     mbar_init_fence();
+    request_stage_tables<TWN>(tab, p.twtab, tabbar);
     tma_prefetch_desc(&map0);
     tma_prefetch_desc(&map1);
   }
-  load_stage_tables<TWN>(tab, p.twtab);  // ends with __syncthreads
+  __syncthreads();
+  pdl_wait();                            // the field buffers are the predecessor's output; the tables above are not
   const int grp = threadIdx.x / MMF_GROUP_THREADS, t = threadIdx.x % MMF_GROUP_THREADS;
   const bool elect = t == 0;
   const int bar = 1 + grp;
@@ -197,6 +210,7 @@ k_cols(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
 
   if (threadIdx.x == 0)
     for (long long tt = 0; tt < S && tt < ntile; ++tt) issue_load(tt);
+  await_stage_tables<TWN>(tabbar);
 
   const int base1 = stage_base<LO1>(t), basel = stage_base<LOL>(t);
   const int c = t & (W - 1);
@@ -262,11 +276,13 @@ __global__ void __launch_bounds__(32, 1) k_perm(const __grid_constant__ CUtensor
   constexpr int S = 3;
   constexpr int TILE_BYTES = (int)sizeof(cpx) << MMF_TILE_LOG;
   uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S * TILE_BYTES);
+  pdl_launch_dependents();
   if (threadIdx.x != 0) return;
 #pragma unroll
   for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
   mbar_init_fence();
   tma_prefetch_desc(&mapn);
+  pdl_wait();
   const int logrt = MMF_TILE_LOG - p.logwb;                 // rows per tile
   const int lognb = p.logn2 - p.logwb;                      // blocks per row
   const int logtb = p.logn1 - logrt;                        // tiles per block
@@ -361,19 +377,23 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
   // The E values of a thread are the same for the 2 nbuf sub-tiles of an item: the first sub-tile takes them from
   // global memory and parks them in tensor memory (64 columns of the thread's own lane), the others read them back
   // from there — no global-load latency, no LSU traffic, no shared memory (none is left).
-  constexpr bool ECACHE = MODE == 0 && !SINGLE;
+  constexpr bool ECACHE = MODE == 0;
   // 4096-point transforms: the exchange between the last two stages goes through tensor memory (tmem_exchange.cuh),
   // 64 more columns per warp
   constexpr bool TMX = LOGN2 == 12;
   constexpr uint32_t WARP_COLS = TMX ? 128 : 64;
   constexpr uint32_t TMEM_COLS = 4 * WARP_COLS;  // 4 warps share a lane quarter
   uint32_t* tmem_word = reinterpret_cast<uint32_t*>(done + G);
+  uint64_t* tabbar = done + G + 1;
+  pdl_launch_dependents();
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
 #pragma unroll
     for (int i = 0; i < G; ++i) mbar_init(&done[i], MMF_GROUP_THREADS);
+    mbar_init(tabbar, 1);
     mbar_init_fence();
+    request_stage_tables<TWN>(tab, p.twtab, tabbar);
   }
   if constexpr (ECACHE || TMX) {
     if (threadIdx.x < 32) {
@@ -382,7 +402,8 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
     }
     tmem_fence_before_sync();
   }
-  load_stage_tables<TWN>(tab, p.twtab);  // ends with __syncthreads
+  __syncthreads();
+  pdl_wait();                            // the field buffers (and, after plan set-up, the E table) come from predecessors
   uint32_t taddr = 0;   // this warp's columns: [0, 64) the E values of the item, [64, 128) the exchange buffer (TMX)
   if constexpr (ECACHE || TMX) {
     tmem_fence_after_sync();
@@ -478,6 +499,7 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
     }
     for (long long tt = 0; tt < S && tt < ntile; ++tt) issue_load(tt);
   }
+  await_stage_tables<TWN>(tabbar);
 
   // Only the tile number stays live across the transforms: geometry is recomputed where it is needed (the table
   // pointer after the forward chain, the store address by the first thread) to keep the 16 values in registers.
@@ -495,11 +517,19 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
       int buf;
       tile_geom(tt, chunk0, buf, item);
       if ((int)item != cached_item) {  // uniform over the group
-        const long long a = item >> (logn1 - LOGB), tau = item & ((1LL << (logn1 - LOGB)) - 1);
-        const cpx* e = p.E + (((a << logn1) + (tau << LOGB) + cht) << LOGN2) + tq;
+        long long ech;  // table chunk of this thread's last-stage values
+        bool live = true;
+        if constexpr (SINGLE) {
+          ech = (chunk0 + cht) >> 1;   // chunk = row, table chunk = mode
+          live = chunk0 + cht < p.nchunks;  // ragged last tile: rows that do not exist (never stored)
+        } else {
+          const long long a = item >> (logn1 - LOGB), tau = item & ((1LL << (logn1 - LOGB)) - 1);
+          ech = (a << logn1) + (tau << LOGB) + cht;
+        }
+        const cpx* e = p.E + (ech << LOGN2) + tq;
         cpx ev[16];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) ev[j] = __ldg(e + (j << (LOGN2 - 4)));
+        for (int j = 0; j < 16; ++j) ev[j] = live ? __ldg(e + (j << (LOGN2 - 4))) : make_double2(1.0, 0.0);
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
           const cpx pr[2] = {ev[2 * c], ev[2 * c + 1]};
@@ -534,15 +564,6 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
             v[8 * hb + 2 * c] = cmul(v[8 * hb + 2 * c], ev[0]);
             v[8 * hb + 2 * c + 1] = cmul(v[8 * hb + 2 * c + 1], ev[1]);
           }
-        }
-      } else {
-        long long chunk0, item;
-        int buf;
-        tile_geom(tt, chunk0, buf, item);
-        if (chunk0 + cht < p.nchunks) {
-          const cpx* e = p.E + (((chunk0 + cht) >> 1) << LOGN2) + tq;  // chunk = row, table chunk = mode
-#pragma unroll
-          for (int j = 0; j < 16; ++j) v[j] = cmul(v[j], __ldg(e + (j << (LOGN2 - 4))));
         }
       }
       if constexpr (TMX) fft12_dit_tm<-1>(v, s, lay, tab, bar, taddr + 64);

@@ -3,6 +3,7 @@
 // there is no CPU fallback.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -133,6 +134,7 @@ struct mmf_plan {
   struct OccEntry { const void* kern; int threads; size_t smem; int occ; };
   std::vector<OccEntry> occ_cache;
   bool dry_run = false;              // launch helpers prepare (attributes, maps) but do not launch
+  bool pdl = true;                   // launch with programmatic stream serialization (async_copy.cuh); MMF_PDL=0 disables
   cudaStream_t cap_stream = nullptr; // capture stream of the step-body graphs
   struct GraphEntry { const void* X; const void* Y; int reps; long long nlaunch; cudaGraphExec_t exec; };
   std::vector<GraphEntry> graphs;
@@ -176,6 +178,27 @@ struct LaunchTimer {
     if (stop) cudaEventRecord(stop, st);
   }
 };
+
+// Every kernel of the propagation paths goes through here: with programmatic stream serialization the grid may start
+// while its predecessor in the stream drains (its prologue — barrier init, tensor-memory allocation, constant tables —
+// overlaps that tail; griddepcontrol.wait in the kernel orders everything that touches the predecessor's output).
+// Off while per-launch events are being recorded (the events must bracket whole kernels).
+template <class... KArgs, class... Args>
+cudaError_t launch_kernel(const mmf_plan* p, void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem,
+                          cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(grid, 1, 1);
+  cfg.blockDim = dim3(block, 1, 1);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = (p->pdl && !p->timing) ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
 
 void clear_events(mmf_plan* p) {
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
@@ -325,9 +348,8 @@ int launch_cols_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cudaStream_t st) {
   long long grid = tiles < p->num_sms ? tiles : p->num_sms;
   if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, DIR == 0 ? KC_COLS_FWD : KC_COLS_INV, 2 * nbuf, st);
-  kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(map0, map1, q);
+  CU(launch_kernel(p, kern, (unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st, map0, map1, q));
   p->launches++;
-  CU(cudaGetLastError());
   return MMF_OK;
 }
 
@@ -367,9 +389,8 @@ int launch_rows_t(mmf_plan* p, cpx* X0, cpx* X1, int nbuf, cpx* OUT, cudaStream_
   long long grid = items < p->num_sms ? items : p->num_sms;
   if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_ROWS, 2 * nbuf, st);
-  kern<<<(unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st>>>(map0, map1, q);
+  CU(launch_kernel(p, kern, (unsigned)grid, MMF_GROUP_THREADS * kGroups, smem, st, map0, map1, q));
   p->launches++;
-  CU(cudaGetLastError());
   return MMF_OK;
 }
 
@@ -424,9 +445,8 @@ int launch_perm(mmf_plan* p, cpx* natural, cpx* blocked, cudaStream_t st) {
   long long grid = tiles < p->num_sms ? tiles : p->num_sms;
   if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_PERM, 2, st);
-  kern<<<(unsigned)grid, 32, smem, st>>>(mapn, q);
+  CU(launch_kernel(p, kern, (unsigned)grid, 32, smem, st, mapn, q));
   p->launches++;
-  CU(cudaGetLastError());
   return MMF_OK;
 }
 int to_tiled(mmf_plan* p, cpx* natural, cpx* tiled, cudaStream_t st) { return launch_perm<0>(p, natural, tiled, st); }
@@ -449,9 +469,8 @@ int launch_nl(mmf_plan* p, cpx* X, cpx* Y, cpx* Z, cpx* W, cudaStream_t st, doub
   const unsigned grid = (unsigned)((p->N + MMF_NL_T - 1) / MMF_NL_T);
   if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_NL_PLAIN + MODE, MODE == NL_PLAIN ? 2 : MODE == NL_STAGE2 ? 3 : MODE == NL_STAGE3 ? 5 : MODE == NL_FINAL ? 3 : 4, st);
-  kern<<<grid, MMF_NL_T * MMF_NL_WARPS, smem, st>>>(q);
+  CU(launch_kernel(p, kern, grid, MMF_NL_T * MMF_NL_WARPS, smem, st, q));
   p->launches++;
-  CU(cudaGetLastError());
   return MMF_OK;
 }
 
@@ -541,9 +560,8 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st, dou
                              : MODE == NLM_AGR_S0 ? 1.25 : MODE == NLM_AGR_IT1 ? 2.25 : MODE == NLM_AGR_ITJ ? 3.25 : 3;
   if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_NLM_PLAIN + MODE, kFields, st);
-  kern<<<(unsigned)grid, threads, smem, st>>>(mapA, mapB, mapC, q);
+  CU(launch_kernel(p, kern, (unsigned)grid, (unsigned)threads, smem, st, mapA, mapB, mapC, q));
   p->launches++;
-  CU(cudaGetLastError());
   return MMF_OK;
 }
 
@@ -596,9 +614,8 @@ int launch_nlg(mmf_plan* p, const cpx* F0, const cpx* F1, const cpx* Hin, cpx* H
   constexpr double kFields = MODE == NLG_PLAIN ? 2 : MODE == NLG_STAGE2 ? 3 : MODE == NLG_STAGE3 ? 5 : 3;
   if (p->dry_run) return MMF_OK;
   LaunchTimer lt(p, KC_NLG_PLAIN + MODE, kFields, st);
-  kern<<<(unsigned)(2 * pairs), 32 * (q.NW + 1), smem, st>>>(mF0, mF1, mHin, mHo0, mHo1, q);
+  CU(launch_kernel(p, kern, (unsigned)(2 * pairs), (unsigned)(32 * (q.NW + 1)), smem, st, mF0, mF1, mHin, mHo0, mHo1, q));
   p->launches++;
-  CU(cudaGetLastError());
   return MMF_OK;
 }
 
@@ -668,6 +685,10 @@ static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, doubl
   p->beta.assign(beta, beta + (size_t)M * K);
   p->kappa.assign(kappa, kappa + KD * KD);
   p->general = general;
+  {
+    const char* e = getenv("MMF_PDL");
+    if (e && e[0] == '0') p->pdl = false;
+  }
   int logn = 0;
   while ((1LL << logn) < N) ++logn;
   p->logn = logn;

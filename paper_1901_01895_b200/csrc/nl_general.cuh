@@ -106,6 +106,7 @@ k_nlg(const __grid_constant__ CUtensorMap mapF0, const __grid_constant__ CUtenso
     tmem_alloc(tmem_word, 512);
   }
   tmem_fence_before_sync();
+  pdl_launch_dependents();
   for (int i = threadIdx.x; i < (int)(2 * pbytes / sizeof(double)); i += blockDim.x) Pb0[i] = 0.0;  // padding rows stay 0
   __syncthreads();
   tmem_fence_after_sync();
@@ -120,6 +121,7 @@ k_nlg(const __grid_constant__ CUtensorMap mapF0, const __grid_constant__ CUtenso
       tma_prefetch_desc(&mapHin);
       tma_prefetch_desc(&mapHo0);
       tma_prefetch_desc(&mapHo1);
+      pdl_wait();   // the fields are the predecessor's output (only this thread touches them in global memory)
       const int own_row = half * M;
       auto store_tile = [&](long long tl, int slot) {
         unsigned char* s = smem_raw + slot * slot_bytes;

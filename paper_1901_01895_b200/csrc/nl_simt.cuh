@@ -1,6 +1,7 @@
 // nl_simt.cuh — the fused nonlinear kernel on the plain FP64 pipe (DFMA), used when M exceeds what the tensor-path
 // kernel of nl_tma.cuh keeps in registers (M > 120).  Rows a4-a7 of the hot-path table.
 #pragma once
+#include "async_copy.cuh"
 #include "fft_core.cuh"
 
 namespace mmf {
@@ -52,6 +53,8 @@ __global__ void __launch_bounds__(MMF_NL_T* MMF_NL_WARPS) k_nl(NlParams p) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* P1 = reinterpret_cast<double*>(smem_raw);
   double* P2 = P1 + (size_t)p.M * MMF_NL_T;
+  pdl_launch_dependents();
+  pdl_wait();   // every thread reads the predecessor's output from global memory
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long tt = (long long)blockIdx.x * MMF_NL_T + lane;
   const bool live = tt < p.N;

@@ -131,6 +131,7 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
     }
     mbar_init_fence();
   }
+  pdl_launch_dependents();
   for (int i = threadIdx.x; i < 2 * 4 * NK * MMF_NLM_PSTRIDE; i += blockDim.x) Pb0[i] = 0.0;  // padding rows stay 0
   __syncthreads();
 
@@ -142,6 +143,7 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
     tma_prefetch_desc(&mapA);
     tma_prefetch_desc(&mapB);
     tma_prefetch_desc(&mapC);
+    pdl_wait();   // the fields are the predecessor's output (only this thread touches global memory)
     // natural-order tile that holds the samples of blocked tile t (ENTER reads it, EXIT writes it)
     auto natural_tile = [&](long long t) -> long long {
       const int u8 = p.logwb - 3;  // log2(tiles per unit of WB columns)
