@@ -108,6 +108,36 @@ int mmf_propagate_host(mmf_plan *plan, void *A_host, void *A_dev_scratch, int ns
 int mmf_propagate_host_batch(mmf_plan *plan, void *const *A_hosts, int nfields, void *A_dev0, void *A_dev1, int nsteps,
                              void *cuda_stream);
 
+/* ROW-SHARDED propagation (sections 4.1-4.3: every process holds whole rows of the signal matrix and
+ * "the squared absolute values have to be shared between the GPUs" once per evaluation of N, four times per step).
+ * A shard plan describes ONE rank: its M_local modes mode0 .. mode0 + M_local - 1 of a fibre with M_total modes.
+ *   beta        host, [M_local][K]: the rank's own modes.
+ *   kappa_rows  host, [M_local][M_total] row-major: rows mode0 .. of the fibre's kappa (all columns).
+ * Workspace (mmf_plan_workspace_bytes): three field buffers of the rank's size (four when N > 4096) + its E table.
+ * One RK4IP step is the sequence below, driven by the caller with ITS collective between powers and apply
+ * (paper_1901_01895_b200/sharded.py does it with torch.distributed; the library itself never communicates):
+ *   mmf_shard_begin(A)                         the rank's rows [2 M_local][N]; A stays attached until mmf_shard_end
+ *   powers(0); all-gather; apply(0)            Y <- h N(A) A                                  (bracket of Eq. 6b)
+ *   per step:  linear(0)                       A_I = D A, k1 = D Y                            (6a), (6b)
+ *              powers(1); all-gather; apply(1) k2 = h N(A_I + k1/2)(A_I + k1/2)               (6c)
+ *              powers(2); all-gather; apply(2) k3 (6d) and the brackets of (6e), (6f)
+ *              linear(1)                       u4 = D(A_I + k3), D(bracket)                   (6e), (6f)
+ *              powers(3); all-gather; apply(3, gain)   A <- gain (D(bracket) + h N(u4) u4 / 6)   (6e), (6f)
+ *              powers(0); all-gather; apply(0) for the next step (not after the last one)
+ *   mmf_shard_end()                            the result is in A
+ * mmf_shard_powers writes rows mode0 .. mode0 + M_local - 1 of P_all (device, [M_total][N] doubles, row-major):
+ *   P_all[b][t] = |u_bx(t)|^2 + |u_by(t)|^2, u the argument of the stage's N; the caller's all-gather fills the other
+ *   rows; mmf_shard_apply reads all of them.  For N > 4096 the sample index t of P_all is the library's internal
+ *   (blocked) order — the same on every rank, since it depends on N only.  stage: 0..3 as listed.
+ * Shard plans accept only the mmf_shard_* calls, mmf_apply_linear and the timing / debug calls. */
+int mmf_plan_create_shard(mmf_plan **out, int M_local, int M_total, int mode0, long long N, double dt, double h,
+                          double alpha, const double *beta, int K, double gamma, const double *kappa_rows);
+int mmf_shard_begin(mmf_plan *plan, void *A_dev, void *cuda_stream);
+int mmf_shard_powers(mmf_plan *plan, int stage, void *P_all_dev, void *cuda_stream);
+int mmf_shard_apply(mmf_plan *plan, int stage, const void *P_all_dev, double gain, void *cuda_stream);
+int mmf_shard_linear(mmf_plan *plan, int which, void *cuda_stream);
+int mmf_shard_end(mmf_plan *plan, void *cuda_stream);
+
 /* Stage-level entry points (each is a row group of the hot path; used by the parity tests).
  * mmf_apply_linear:    X <- exp(h/2 L) X  (Eq. 6a: transform, multiply by exp(h/2 L_a(w_k)), transform back), in place.
  * mmf_apply_nonlinear: OUT <- h N(U) U = i h gamma (sum_b kappa_ab |U_b|^2) U_a   (Eq. 1 / the bracket of Eq. 6b).

@@ -14,7 +14,8 @@ LIB_PATH = os.path.join(_HERE, "libmmf_b200.so")
 MMF_OK, MMF_EINVAL, MMF_ENOMEM, MMF_ECUDA = 0, -1, -2, -3
 
 # every symbol include/mmf.h declares (tests check that the built library exports all of them)
-SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate", "mmf_propagate_ssfm",
+SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_create_shard", "mmf_shard_begin", "mmf_shard_powers",
+           "mmf_shard_apply", "mmf_shard_linear", "mmf_shard_end", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate", "mmf_propagate_ssfm",
            "mmf_propagate_ssfm_agrawal", "mmf_propagate_spans",
            "mmf_propagate_host", "mmf_propagate_host_batch", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
            "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_set_timing", "mmf_kernel_class_count",
@@ -43,6 +44,18 @@ def lib():
     L.mmf_plan_create.restype = i
     L.mmf_plan_create_general.argtypes = [ctypes.POINTER(vp), i, ll, d, d, d, dp, i, d, dp]
     L.mmf_plan_create_general.restype = i
+    L.mmf_plan_create_shard.argtypes = [ctypes.POINTER(vp), i, i, i, ll, d, d, d, dp, i, d, dp]
+    L.mmf_plan_create_shard.restype = i
+    L.mmf_shard_begin.argtypes = [vp, vp, vp]
+    L.mmf_shard_begin.restype = i
+    L.mmf_shard_powers.argtypes = [vp, i, vp, vp]
+    L.mmf_shard_powers.restype = i
+    L.mmf_shard_apply.argtypes = [vp, i, vp, d, vp]
+    L.mmf_shard_apply.restype = i
+    L.mmf_shard_linear.argtypes = [vp, i, vp]
+    L.mmf_shard_linear.restype = i
+    L.mmf_shard_end.argtypes = [vp, vp]
+    L.mmf_shard_end.restype = i
     L.mmf_plan_workspace_bytes.argtypes = [vp]
     L.mmf_plan_workspace_bytes.restype = sz
     L.mmf_plan_set_workspace.argtypes = [vp, vp, sz, vp]
@@ -106,21 +119,29 @@ def _stream_ptr(stream=None):
 class Plan:
     """mmf_plan_create / mmf_plan_set_workspace / mmf_propagate / mmf_plan_destroy with torch-owned buffers."""
 
-    def __init__(self, M, N, dt, h, alpha, beta, gamma, kappa, device="cuda:0", general=False):
-        """general=True: kappa is the [2M][2M] per-polarisation matrix (mmf_plan_create_general)."""
+    def __init__(self, M, N, dt, h, alpha, beta, gamma, kappa, device="cuda:0", general=False, shard=None):
+        """general=True: kappa is the [2M][2M] per-polarisation matrix (mmf_plan_create_general).
+        shard=(M_total, mode0): a row-shard plan (mmf_plan_create_shard): M own modes, kappa = their [M][M_total] rows."""
         import torch
         L = lib()
         self.M, self.N = int(M), int(N)
         beta = np.ascontiguousarray(beta, dtype=np.float64).reshape(self.M, -1)
         kd = 2 * self.M if general else self.M
-        kappa = np.ascontiguousarray(kappa, dtype=np.float64).reshape(kd, kd)
+        kc = int(shard[0]) if shard is not None else kd
+        kappa = np.ascontiguousarray(kappa, dtype=np.float64).reshape(kd, kc)
         self._h = ctypes.c_void_p()
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         dp = ctypes.POINTER(ctypes.c_double)
-        create = L.mmf_plan_create_general if general else L.mmf_plan_create
-        rc = create(ctypes.byref(self._h), self.M, self.N, float(dt), float(h), float(alpha),
-                    beta.ctypes.data_as(dp), beta.shape[1], float(gamma), kappa.ctypes.data_as(dp))
+        if shard is not None:
+            self.M_total, self.mode0 = int(shard[0]), int(shard[1])
+            rc = L.mmf_plan_create_shard(ctypes.byref(self._h), self.M, self.M_total, self.mode0, self.N, float(dt), float(h),
+                                         float(alpha), beta.ctypes.data_as(dp), beta.shape[1], float(gamma),
+                                         kappa.ctypes.data_as(dp))
+        else:
+            create = L.mmf_plan_create_general if general else L.mmf_plan_create
+            rc = create(ctypes.byref(self._h), self.M, self.N, float(dt), float(h), float(alpha),
+                        beta.ctypes.data_as(dp), beta.shape[1], float(gamma), kappa.ctypes.data_as(dp))
         _check(rc, "mmf_plan_create")
         nbytes = L.mmf_plan_workspace_bytes(self._h)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
@@ -157,6 +178,30 @@ class Plan:
         """In-place SSFM-Agrawal propagation (symmetric split step, iterative trapezoidal nonlinear part)."""
         _check(lib().mmf_propagate_ssfm_agrawal(self._h, self._field_ptr(A), int(nsteps), int(niter),
                                                 _stream_ptr(stream)), "mmf_propagate_ssfm_agrawal")
+
+    # -- row-sharded propagation: the stage calls paper_1901_01895_b200/sharded.py sequences around its all-gather
+    def shard_begin(self, A, stream=None):
+        _check(lib().mmf_shard_begin(self._h, self._field_ptr(A), _stream_ptr(stream)), "mmf_shard_begin")
+
+    def shard_powers(self, stage, P_all, stream=None):
+        import torch
+        assert P_all.is_cuda and P_all.dtype == torch.float64 and P_all.is_contiguous()
+        assert tuple(P_all.shape) == (self.M_total, self.N)
+        _check(lib().mmf_shard_powers(self._h, int(stage), ctypes.c_void_p(P_all.data_ptr()), _stream_ptr(stream)),
+               "mmf_shard_powers")
+
+    def shard_apply(self, stage, P_all, gain=1.0, stream=None):
+        import torch
+        assert P_all.is_cuda and P_all.dtype == torch.float64 and P_all.is_contiguous()
+        assert tuple(P_all.shape) == (self.M_total, self.N)
+        _check(lib().mmf_shard_apply(self._h, int(stage), ctypes.c_void_p(P_all.data_ptr()), float(gain),
+                                     _stream_ptr(stream)), "mmf_shard_apply")
+
+    def shard_linear(self, which, stream=None):
+        _check(lib().mmf_shard_linear(self._h, int(which), _stream_ptr(stream)), "mmf_shard_linear")
+
+    def shard_end(self, stream=None):
+        _check(lib().mmf_shard_end(self._h, _stream_ptr(stream)), "mmf_shard_end")
 
     def propagate_host(self, A_host, A_scratch, nsteps, stream=None):
         """A_host: pinned torch complex128 CPU tensor (2M, N); A_scratch: CUDA tensor of the same shape."""

@@ -13,6 +13,7 @@
 #include "nl_tma.cuh"
 #include "nl_simt.cuh"
 #include "nl_general.cuh"
+#include "nl_shard.cuh"
 
 using namespace mmf;
 
@@ -113,6 +114,10 @@ struct mmf_plan {
   int M = 0, K = 0, logn = 0, logn1 = 0, logn2 = 0;
   int nlm_nk = -1;   // k-steps of the tensor-path nonlinear kernel; -1: M too large, legacy kernels (4 buffers)
   bool general = false;  // kappa is the general [2M][2M] per-polarisation matrix (k_nlg, four-buffer plan)
+  // row-sharded plan (mmf_plan_create_shard): M = the rank's own modes, kappa = its [M][M_total] rows
+  int M_total = 0, mode0 = 0;
+  cpx* shard_X = nullptr;   // the rank's field while a sharded propagation is open (mmf_shard_begin .. mmf_shard_end)
+  void* shard_A = nullptr;
   int num_sms = 148;
   int device = 0;    // the device the plan's tables live on; every call must be made with it current
   long long N = 0;
@@ -151,12 +156,13 @@ namespace {
 // ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
 enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
        KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_NLM_ENTER, KC_NLM_EXIT, KC_NLM_AGR_S0,
-       KC_NLM_AGR_IT1, KC_NLM_AGR_ITJ, KC_PERM, KC_NLG_PLAIN, KC_NLG_STAGE2, KC_NLG_STAGE3, KC_NLG_FINAL, KC_COUNT };
+       KC_NLM_AGR_IT1, KC_NLM_AGR_ITJ, KC_PERM, KC_NLG_PLAIN, KC_NLG_STAGE2, KC_NLG_STAGE3, KC_NLG_FINAL, KC_SHARD_POW, KC_SHARD_APPLY, KC_COUNT };
 const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
                                         "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>", "k_nlm<plain>",
                                         "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>", "k_nlm<enter>",
                                         "k_nlm<exit>", "k_nlm<agr_s0>", "k_nlm<agr_it1>", "k_nlm<agr_itj>", "k_perm",
-                                        "k_nlg<plain>", "k_nlg<stage2>", "k_nlg<stage3>", "k_nlg<final>"};
+                                        "k_nlg<plain>", "k_nlg<stage2>", "k_nlg<stage3>", "k_nlg<final>", "k_shard_pow",
+                                        "k_shard_apply"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
 struct LaunchTimer {
@@ -640,6 +646,40 @@ void free_tables(mmf_plan* p) {
 
 }  // namespace
 
+namespace {
+template <int STAGE>
+int launch_shard(mmf_plan* p, bool pow, double* P_all, double gain, cudaStream_t st) {
+  ShardParams q;
+  q.X = p->shard_X; q.Y = p->Y; q.Z = p->Z; q.W = p->W;
+  q.kappa_rows = p->d_kappa; q.P_all = P_all;
+  q.hg = p->h * p->gamma; q.gain = gain;
+  q.M_local = p->M; q.M_total = p->M_total; q.mode0 = p->mode0; q.N = p->N;
+  const unsigned grid = (unsigned)((p->N + MMF_SH_T - 1) / MMF_SH_T);
+  if (pow) {
+    LaunchTimer lt(p, KC_SHARD_POW, STAGE == SH_PLAIN || STAGE == SH_FINAL ? 1.0 : 2.0, st);
+    CU(launch_kernel(p, k_shard_pow<STAGE>, grid, MMF_SH_T * MMF_SH_WARPS, 0, st, q));
+  } else {
+    const size_t smem = sizeof(double) * (size_t)p->M_total * MMF_SH_T;
+    auto kern = k_shard_apply<STAGE>;
+    MMF_ENSURE_SMEM(kern, smem);
+    LaunchTimer lt(p, KC_SHARD_APPLY, STAGE == SH_PLAIN ? 2 : STAGE == SH_STAGE2 ? 3 : STAGE == SH_STAGE3 ? 5 : 3, st);
+    CU(launch_kernel(p, kern, grid, MMF_SH_T * MMF_SH_WARPS, smem, st, q));
+  }
+  p->launches++;
+  return MMF_OK;
+}
+int shard_stage(mmf_plan* p, int stage, bool pow, double* P_all, double gain, cudaStream_t st) {
+  switch (stage) {
+    case SH_PLAIN: return launch_shard<SH_PLAIN>(p, pow, P_all, gain, st);
+    case SH_STAGE2: return launch_shard<SH_STAGE2>(p, pow, P_all, gain, st);
+    case SH_STAGE3: return launch_shard<SH_STAGE3>(p, pow, P_all, gain, st);
+    case SH_FINAL: return launch_shard<SH_FINAL>(p, pow, P_all, gain, st);
+    default: return MMF_EINVAL;
+  }
+}
+bool shard_ready(const mmf_plan* p) { return p && p->M_total > 0 && p->ws && on_plan_device(p); }
+}  // namespace
+
 extern "C" {
 
 const char* mmf_version(void) { return "mmf-b200 0.1"; }
@@ -655,7 +695,7 @@ const char* mmf_status_string(int status) {
 }
 
 static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, double h, double alpha, const double* beta,
-                            int K, double gamma, const double* kappa, bool general);
+                            int K, double gamma, const double* kappa, bool general, int M_total = 0, int mode0 = 0);
 
 int mmf_plan_create(mmf_plan** out, int M, long long N, double dt, double h, double alpha, const double* beta, int K,
                     double gamma, const double* kappa) {
@@ -667,24 +707,34 @@ int mmf_plan_create_general(mmf_plan** out, int M, long long N, double dt, doubl
   return plan_create_impl(out, M, N, dt, h, alpha, beta, K, gamma, kappa2, true);
 }
 
+int mmf_plan_create_shard(mmf_plan** out, int M_local, int M_total, int mode0, long long N, double dt, double h,
+                          double alpha, const double* beta, int K, double gamma, const double* kappa_rows) {
+  if (M_local < 1 || mode0 < 0 || M_total < M_local || mode0 + M_local > M_total) return MMF_EINVAL;
+  return plan_create_impl(out, M_local, N, dt, h, alpha, beta, K, gamma, kappa_rows, false, M_total, mode0);
+}
+
 static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, double h, double alpha, const double* beta,
-                            int K, double gamma, const double* kappa, bool general) {
+                            int K, double gamma, const double* kappa, bool general, int M_total, int mode0) {
   if (!out) return MMF_EINVAL;
   *out = nullptr;
   if (!beta || !kappa || M < 1 || K < 1 || K > MMF_MAXK) return MMF_EINVAL;
   if (N < 16 || N > (1LL << 24) || (N & (N - 1)) != 0) return MMF_EINVAL;
   if (!(dt > 0) || !std::isfinite(dt) || !std::isfinite(h) || !std::isfinite(alpha) || !std::isfinite(gamma))
     return MMF_EINVAL;
-  const size_t KD = general ? 2 * (size_t)M : (size_t)M;   // kappa is KD x KD
+  const bool shard = M_total > 0;
+  const size_t KD = general ? 2 * (size_t)M : (size_t)M;   // kappa is KD x KC
+  const size_t KC = shard ? (size_t)M_total : KD;
   if (general && M > MMF_NLG_MAXM) return MMF_EINVAL;       // the general kernel keeps an M x 2M slab in tensor memory
-  if (!finite_all(beta, (size_t)M * K) || !finite_all(kappa, KD * KD)) return MMF_EINVAL;
-  if (sizeof(double) * 2 * (size_t)M * MMF_NL_T > 227 * 1024) return MMF_EINVAL;  // mode-power tile must fit one SM
+  if (!finite_all(beta, (size_t)M * K) || !finite_all(kappa, KD * KC)) return MMF_EINVAL;
+  if (sizeof(double) * 2 * KC * MMF_NL_T > 227 * 1024) return MMF_EINVAL;  // mode-power tile must fit one SM
   mmf_plan* p = new (std::nothrow) mmf_plan;
   if (!p) return MMF_ENOMEM;
   p->M = M; p->K = K; p->N = N; p->dt = dt; p->h = h; p->alpha = alpha; p->gamma = gamma;
   p->beta.assign(beta, beta + (size_t)M * K);
-  p->kappa.assign(kappa, kappa + KD * KD);
+  p->kappa.assign(kappa, kappa + KD * KC);
   p->general = general;
+  p->M_total = M_total;
+  p->mode0 = mode0;
   {
     const char* e = getenv("MMF_PDL");
     if (e && e[0] == '0') p->pdl = false;
@@ -700,7 +750,7 @@ static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, doubl
   else if (logn <= 22) p->logn1 = 10;
   else p->logn1 = 12;
   p->logn2 = logn - p->logn1;
-  p->nlm_nk = (!general && M <= MMF_NLM_MAXM) ? nlm_pick_nk(M) : -1;
+  p->nlm_nk = (!general && !shard && M <= MMF_NLM_MAXM) ? nlm_pick_nk(M) : -1;   // shard plans: four-buffer plan
   {
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) == cudaSuccess) p->device = dev;
@@ -709,9 +759,9 @@ static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, doubl
   p->field_bytes = sizeof(cpx) * 2 * (size_t)M * (size_t)N;
   int rc = MMF_OK;
   do {
-    cudaError_t e = cudaMalloc((void**)&p->d_kappa, sizeof(double) * KD * KD);
+    cudaError_t e = cudaMalloc((void**)&p->d_kappa, sizeof(double) * KD * KC);
     if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MMF_ENOMEM : cuda_fail(e); break; }
-    e = cudaMemcpy(p->d_kappa, kappa, sizeof(double) * KD * KD, cudaMemcpyHostToDevice);
+    e = cudaMemcpy(p->d_kappa, kappa, sizeof(double) * KD * KC, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { rc = cuda_fail(e); break; }
     if ((rc = upload_stage_tables(&p->d_tw2, p->logn2)) != MMF_OK) break;
     if (p->logn1 > 0) {
@@ -895,7 +945,7 @@ int run_bodies(mmf_plan* p, cpx* X, cpx* Y, int nbody, cudaStream_t st) {
 // nsteps RK4IP steps; span > 0: after every span-th step the new field is multiplied by `gain` (lumped amplifier)
 static int propagate_impl(mmf_plan* p, void* A_dev, int nsteps, int span, double gain, void* cuda_stream) {
   if (!p || !A_dev || nsteps < 0 || ((size_t)A_dev & 15) != 0) return MMF_EINVAL;
-  if (!p->ws || !on_plan_device(p)) return MMF_EINVAL;
+  if (!p->ws || !on_plan_device(p) || p->M_total > 0) return MMF_EINVAL;   // shard plans: the mmf_shard_* calls
   if (nsteps == 0) return MMF_OK;
   auto gain_of = [&](int s) { return (span > 0 && (s + 1) % span == 0) ? gain : 1.0; };   // gain applied by step s
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -1119,6 +1169,7 @@ int mmf_apply_linear(mmf_plan* p, void* X_dev, void* cuda_stream) {
 
 int mmf_apply_nonlinear(mmf_plan* p, const void* U_dev, void* OUT_dev, void* cuda_stream) {
   if (!p || !U_dev || !OUT_dev || (((size_t)U_dev | (size_t)OUT_dev) & 15) != 0 || !on_plan_device(p)) return MMF_EINVAL;
+  if (p->M_total > 0) return MMF_EINVAL;   // a shard sees only its own rows
   if (p->general) {
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (U_dev != OUT_dev) return launch_nlg<NLG_PLAIN>(p, (const cpx*)U_dev, nullptr, nullptr, (cpx*)OUT_dev, nullptr, st);
@@ -1130,6 +1181,45 @@ int mmf_apply_nonlinear(mmf_plan* p, const void* U_dev, void* OUT_dev, void* cud
   }
   if (p->nlm_nk > 0) return launch_nlm<NLM_PLAIN>(p, (const cpx*)U_dev, (cpx*)OUT_dev, (cudaStream_t)cuda_stream);
   return launch_nl<NL_PLAIN>(p, (cpx*)U_dev, (cpx*)OUT_dev, nullptr, nullptr, (cudaStream_t)cuda_stream);
+}
+
+// ---- row-sharded propagation: stage entry points, sequenced by paper_1901_01895_b200/sharded.py ----
+
+int mmf_shard_begin(mmf_plan* p, void* A_dev, void* cuda_stream) {
+  if (!shard_ready(p) || !A_dev || ((size_t)A_dev & 15) != 0 || p->shard_A) return MMF_EINVAL;
+  p->shard_A = A_dev;
+  p->shard_X = (cpx*)A_dev;
+  if (p->logn1 > 0) {   // N > 4096: the rank's rows go to the blocked order the transform kernels work in
+    const int rc = to_tiled(p, (cpx*)A_dev, p->V, (cudaStream_t)cuda_stream);
+    if (rc != MMF_OK) { p->shard_A = nullptr; return rc; }
+    p->shard_X = p->V;
+  }
+  return MMF_OK;
+}
+
+int mmf_shard_powers(mmf_plan* p, int stage, void* P_all_dev, void* cuda_stream) {
+  if (!shard_ready(p) || !p->shard_A || !P_all_dev || ((size_t)P_all_dev & 7) != 0) return MMF_EINVAL;
+  return shard_stage(p, stage, true, (double*)P_all_dev, 1.0, (cudaStream_t)cuda_stream);
+}
+
+int mmf_shard_apply(mmf_plan* p, int stage, const void* P_all_dev, double gain, void* cuda_stream) {
+  if (!shard_ready(p) || !p->shard_A || !P_all_dev || ((size_t)P_all_dev & 7) != 0 || !std::isfinite(gain)) return MMF_EINVAL;
+  return shard_stage(p, stage, false, (double*)P_all_dev, gain, (cudaStream_t)cuda_stream);
+}
+
+int mmf_shard_linear(mmf_plan* p, int which, void* cuda_stream) {
+  if (!shard_ready(p) || !p->shard_A || which < 0 || which > 1) return MMF_EINVAL;
+  return which == 0 ? apply_D(p, p->shard_X, p->Y, 2, (cudaStream_t)cuda_stream)     // (6a) A_I, (6b) k1
+                    : apply_D(p, p->W, p->Z, 2, (cudaStream_t)cuda_stream);           // (6e) argument, (6f) first term
+}
+
+int mmf_shard_end(mmf_plan* p, void* cuda_stream) {
+  if (!shard_ready(p) || !p->shard_A) return MMF_EINVAL;
+  int rc = MMF_OK;
+  if (p->logn1 > 0) rc = to_natural(p, p->shard_X, (cpx*)p->shard_A, (cudaStream_t)cuda_stream);
+  p->shard_A = nullptr;
+  p->shard_X = nullptr;
+  return rc;
 }
 
 int mmf_debug_forward(mmf_plan* p, void* X_dev, void* SPEC_dev, void* cuda_stream) {
