@@ -327,14 +327,22 @@ def run_mmf(args):
     nthreads = max(1, len(os.sched_getaffinity(0)) // max(1, world))
     fill_field(p, H.numpy(), nthreads)
     log("[bench] input generated in %.1f s" % (time.perf_counter() - t0))
-    X = torch.empty((p.R, p.N), dtype=torch.complex128, device=dev)
+    general = args.kappa == "general"
+    shard = None
+    if args.shard:
+        # row shards: this rank keeps modes mode0 .. mode0 + m - 1 and all-gathers the mode powers
+        from paper_1901_01895_b200 import sharded
+        assert args.method == "rk4ip" and not general, "--shard: rk4ip with the Manakov kappa"
+        mode0, m, beta_l, kappa_rows = sharded.shard_arguments(p.beta, p.kappa, rank, world)
+        H = H[2 * mode0:2 * (mode0 + m)]
+        shard = sharded.CudaShardStages(p.M, mode0, p.N, p.dt, p.h, p.alpha, beta_l, p.gamma, kappa_rows, device=dev)
+    X = torch.empty(tuple(H.shape), dtype=torch.complex128, device=dev)
     X.copy_(H)
-    if world > 1:                                    # replicas: a launch-power sweep, one power per rank
+    if world > 1 and shard is None:                  # replicas: a launch-power sweep, one power per rank
         X *= replicas.amplitude_scale(rank, world)
         H.copy_(X)
-    general = args.kappa == "general"
-    plan = binding.Plan(p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa_general() if general else p.kappa,
-                        device=dev, general=general)
+    plan = shard.plan if shard is not None else binding.Plan(
+        p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa_general() if general else p.kappa, device=dev, general=general)
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -345,6 +353,9 @@ def run_mmf(args):
     # ---- warm-up (W untimed steps), then K timed steps, field resident in HBM ----
     advance = {"rk4ip": plan.propagate, "ssfm": plan.propagate_ssfm,
                "agrawal": lambda X_, n_: plan.propagate_ssfm_agrawal(X_, n_, niter=args.niter)}[args.method]
+    if shard is not None:
+        def advance(X_, n_):
+            sharded.propagate(shard, X_, n_, lambda: sharded.all_gather_rows(shard.P_all, shard.mode0, shard.M_local, dist))
     advance(X, args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
@@ -370,7 +381,7 @@ def run_mmf(args):
     kern = plan.get_timing()
     plan.set_timing(False)
     clocks = sampler.stop()
-    _, ms, value = replicas.whole_job(p.R * p.N * args.steps, ms, dist, dev)
+    _, ms, value = replicas.whole_job(X.shape[0] * p.N * args.steps, ms, dist, dev)
     assert bool(torch.isfinite(X.view(torch.float64)).all()), "propagated field is not finite"
 
     # ---- end to end: host buffers in, host buffers out, through the C ABI ----
@@ -379,7 +390,7 @@ def run_mmf(args):
     #     field i - 1 comes out while field i propagates.  (b) is the throughput figure; (a) is reported beside it.
     barrier()
     e0.record(stream)
-    if args.method == "rk4ip":
+    if args.method == "rk4ip" and shard is None:
         plan.propagate_host(H, X, args.steps)       # H2D copy, K steps, D2H copy, stream synchronised inside
     else:                                           # no host entry point for the split steps: same copies by hand
         X.copy_(H, non_blocking=True)
@@ -388,9 +399,9 @@ def run_mmf(args):
     e1.record(stream)
     barrier()
     ms_single = e0.elapsed_time(e1)                 # device clock over the whole call
-    _, ms_single, single_value = replicas.whole_job(p.R * p.N * args.steps, ms_single, dist, dev)
+    _, ms_single, single_value = replicas.whole_job(X.shape[0] * p.N * args.steps, ms_single, dist, dev)
     nbatch, ms_e2e, e2e_value = 1, ms_single, single_value
-    if args.method == "rk4ip" and args.e2e_batch > 1:
+    if args.method == "rk4ip" and args.e2e_batch > 1 and shard is None:
         _, avail = host_description()
         free_dev = torch.cuda.mem_get_info(dev)[0]
         nbatch = args.e2e_batch
@@ -417,7 +428,7 @@ def run_mmf(args):
 
     # ---- roofline of the dominant kernel (largest summed device time in the timed region) ----
     peak, peak_src = load_peaks()
-    full_cfg = args.modes is None and args.logn is None and args.method == "rk4ip" and not general
+    full_cfg = args.modes is None and args.logn is None and args.method == "rk4ip" and not general and shard is None
     roof = None
     breakdown = []
     tot_kernel_ms = sum(k["total_ms"] for k in kern) or 1.0
@@ -463,7 +474,11 @@ def run_mmf(args):
                     "avg_launch_ms": avg, "hbm": {"achieved": gb, "peak": peak, "unit": "GB/s", "frac": gb / peak,
                                                   "alg_bytes_per_launch": topg["alg_bytes_per_launch"]}}
     # whole-step roofline: B_alg = 36 F (three-pass transforms) or 20 F (rows fit on chip)
-    if args.method == "rk4ip":
+    if shard is not None:
+        # per rank (its rows: F / world): transforms 24 F_r (8 on chip); powers kernels read 6 F_r and write 4 x F_r / 4;
+        # apply kernels 13 F_r (four-buffer plan, one N per pass) and read the gathered powers 4 x world x F_r / 4
+        balg = ((24 if p.N > 4096 else 8) + 20 + world) * F / world
+    elif args.method == "rk4ip":
         balg = (36 if p.N > 4096 else 20) * F
     elif args.method == "agrawal":                  # (1 + niter) D on one buffer + S0 (1.25 F), IT1 (2.25 F), ITJ (3.25 F)
         balg = ((1 + args.niter) * (6 if p.N > 4096 else 2) + 3.5 + 3.25 * (args.niter - 1)) * F
@@ -518,12 +533,14 @@ def run_mmf(args):
                "single_core": single, "cpu_model": model, "mem_available_GiB": avail}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if shard is not None else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_string(p) + (" [general 2M x 2M kappa]" if general else ""),
                        "method": args.method, "kappa": args.kappa, "l2": "field copy %.1f GiB >> 126 MB L2 (no flush needed)"
                        % (F / 2 ** 30) if F > 4 * 126e6 else "working set near/below L2 size: L2-resident",
-                       "parallelism": "replicas x%d (launch-power sweep, no collective)" % world},
+                       "parallelism": ("row shards x%d (PAPER.md:99-168: whole rows per rank, all-gather of the mode powers 4x per "
+                                       "step, NCCL)" % world) if shard is not None else
+                                      "replicas x%d (launch-power sweep, no collective)" % world},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": F / args.steps,
                     "d2h_bytes_per_step": F / args.steps, "ms_per_call": ms_e2e, "fields_per_call": nbatch,
@@ -555,6 +572,9 @@ def main():
     ap.add_argument("--kappa", default="manakov", choices=["manakov", "general"],
                     help="manakov: kappa [M][M] of Eq. 1 (the headline path); general: the paper's [2M][2M] per-polarisation "
                          "matrix (PAPER.md:176; rk4ip only)")
+    ap.add_argument("--shard", action="store_true",
+                    help="row-sharded path (SURVEY.md NEXT-3): every rank propagates M / world modes and all-gathers the mode "
+                         "powers; with one GPU it measures the split kernels alone")
     ap.add_argument("--modes", type=int, default=None, help="override the config's mode count M (extra data points)")
     ap.add_argument("--logn", type=int, default=None, help="override the config's N = 2^logn (extra data points)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

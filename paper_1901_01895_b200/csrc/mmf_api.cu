@@ -659,11 +659,18 @@ int launch_shard(mmf_plan* p, bool pow, double* P_all, double gain, cudaStream_t
     LaunchTimer lt(p, KC_SHARD_POW, STAGE == SH_PLAIN || STAGE == SH_FINAL ? 1.0 : 2.0, st);
     CU(launch_kernel(p, k_shard_pow<STAGE>, grid, MMF_SH_T * MMF_SH_WARPS, 0, st, q));
   } else {
-    const size_t smem = sizeof(double) * (size_t)p->M_total * MMF_SH_T;
+    const size_t smem = shard_apply_smem_bytes(p->M, p->M_total);
+    if (smem > 227 * 1024) return MMF_EINVAL;
     auto kern = k_shard_apply<STAGE>;
     MMF_ENSURE_SMEM(kern, smem);
+    int occ = 1;
+    int rc = cached_occupancy(p, kern, MMF_SH_T * MMF_SH_WARPS, smem, &occ);
+    if (rc != MMF_OK) return rc;
+    if (occ < 1) return MMF_EINVAL;
+    unsigned pgrid = (unsigned)(p->num_sms * occ);   // persistent: kappa goes to shared memory once per CTA
+    if (pgrid > grid) pgrid = grid;
     LaunchTimer lt(p, KC_SHARD_APPLY, STAGE == SH_PLAIN ? 2 : STAGE == SH_STAGE2 ? 3 : STAGE == SH_STAGE3 ? 5 : 3, st);
-    CU(launch_kernel(p, kern, grid, MMF_SH_T * MMF_SH_WARPS, smem, st, q));
+    CU(launch_kernel(p, kern, pgrid, MMF_SH_T * MMF_SH_WARPS, smem, st, q));
   }
   p->launches++;
   return MMF_OK;

@@ -13,7 +13,7 @@
 // Stages: 0 PLAIN  Y <- NL(X);  1 STAGE2  Z <- NL(X + Y/2);  2 STAGE3  k3 = NL(X + Z/2), W <- X + k3,
 //         Z <- X + Y/6 + Z/3 + k3/3;  3 FINAL  X <- gain (Z + NL(W)/6).
 // Layout: lane = time sample (32 consecutive samples: 512-byte row segments of the fields, 256-byte segments of P),
-// warps stride over the modes; the contraction runs on the plain fp64 pipe with P staged in shared memory.  The path is
+// warps stride over the modes; the contraction runs on the plain fp64 pipe with P and the kappa rows in shared memory.  The path is
 // bound by the collective (M_total N 8 bytes per evaluation), not by these kernels.
 #pragma once
 #include "async_copy.cuh"
@@ -36,7 +36,7 @@ struct ShardParams {
 };
 
 #define MMF_SH_T 32
-#define MMF_SH_WARPS 8
+#define MMF_SH_WARPS 16
 
 template <int STAGE>
 __device__ __forceinline__ cpx shard_arg(const ShardParams& p, long long i) {
@@ -53,7 +53,7 @@ __device__ __forceinline__ cpx shard_arg(const ShardParams& p, long long i) {
   }
 }
 
-// grid = ceil(N / 32), block = 256
+// grid = ceil(N / 32), block = 512
 template <int STAGE>
 __global__ void __launch_bounds__(MMF_SH_T* MMF_SH_WARPS) k_shard_pow(ShardParams p) {
   pdl_launch_dependents();
@@ -67,41 +67,95 @@ __global__ void __launch_bounds__(MMF_SH_T* MMF_SH_WARPS) k_shard_pow(ShardParam
   }
 }
 
-// grid = ceil(N / 32), block = 256, dynamic shared memory = M_total * 32 doubles
+// Persistent: grid = a multiple of the SM count, every CTA walks the 32-sample tiles blockIdx.x, + gridDim.x, ...
+// block = 512 (16 warps; lane = sample).  Dynamic shared memory: the rank's kappa rows TRANSPOSED and padded,
+// ks[b][a] (a < MP = M_local rounded up to 4; loaded once per CTA), the power tile P[b][32] and the result S[a][32].
+// Three phases per tile, so that the global loads of a phase are all in flight together (the kernel is bound by
+// memory latency otherwise: it has few warps per SM):
+//   1. P tile <- P_all (coalesced 256-byte rows);
+//   2. S = kappa_rows * P from shared memory only; a warp computes FOUR modes at a time: per column b one read of
+//      P[b][lane] and two broadcast 16-byte reads of ks[b][a..a+3] feed four FMAs;
+//   3. the stage sums, four field rows per warp at a time: all loads of the four rows first, then the arithmetic.
+__host__ __device__ inline size_t shard_apply_smem_bytes(int M_local, int M_total) {
+  const int MP = (M_local + 3) & ~3;
+  return sizeof(double) * ((size_t)M_total * MP + (size_t)M_total * MMF_SH_T + (size_t)MP * MMF_SH_T);
+}
 template <int STAGE>
 __global__ void __launch_bounds__(MMF_SH_T* MMF_SH_WARPS) k_shard_apply(ShardParams p) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
-  double* P = reinterpret_cast<double*>(smem_raw);
+  const int MP = (p.M_local + 3) & ~3;
+  double* ks = reinterpret_cast<double*>(smem_raw);          // [M_total][MP]
+  double* P = ks + (size_t)p.M_total * MP;                    // [M_total][32]
+  double* Ss = P + (size_t)p.M_total * MMF_SH_T;              // [MP][32]
   pdl_launch_dependents();
+  for (int i = threadIdx.x; i < p.M_total * MP; i += blockDim.x) {
+    const int b = i / MP, a = i - b * MP;
+    ks[i] = a < p.M_local ? p.kappa_rows[(long long)a * p.M_total + b] : 0.0;   // kappa: a constant table
+  }
   pdl_wait();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long long tt = (long long)blockIdx.x * MMF_SH_T + lane;
-  const bool live = tt < p.N;
-  for (int b = warp; b < p.M_total; b += MMF_SH_WARPS) P[b * MMF_SH_T + lane] = live ? p.P_all[(long long)b * p.N + tt] : 0.0;
-  __syncthreads();
   const double third = 1.0 / 3.0, sixth = 1.0 / 6.0;
-  for (int a = warp; a < p.M_local; a += MMF_SH_WARPS) {
-    double S = 0.0;
-    const double* kr = p.kappa_rows + (long long)a * p.M_total;
-    for (int b = 0; b < p.M_total; ++b) S = fma(__ldg(kr + b), P[b * MMF_SH_T + lane], S);
-    const double g = p.hg * S;
-    if (!live) continue;
+  const int R = 2 * p.M_local;
+  constexpr int U = 4;   // field rows per warp and batch in phase 3
+  const long long ntile = (p.N + MMF_SH_T - 1) / MMF_SH_T;
+  for (long long tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
+    const long long tt = tile * MMF_SH_T + lane;
+    const bool live = tt < p.N;
+    __syncthreads();   // the previous tile's P and S are no longer read (and, first time round, ks is complete)
+    for (int b = warp; b < p.M_total; b += MMF_SH_WARPS) P[b * MMF_SH_T + lane] = live ? p.P_all[(long long)b * p.N + tt] : 0.0;
+    __syncthreads();
+    for (int a0 = 4 * warp; a0 < p.M_local; a0 += 4 * MMF_SH_WARPS) {
+      double S[4] = {0.0, 0.0, 0.0, 0.0};
+      const double* kc = ks + a0;
+#pragma unroll 4
+      for (int b = 0; b < p.M_total; ++b) {
+        const double pb = P[b * MMF_SH_T + lane];
+        const double2 k01 = *reinterpret_cast<const double2*>(kc + (size_t)b * MP);
+        const double2 k23 = *reinterpret_cast<const double2*>(kc + (size_t)b * MP + 2);
+        S[0] = fma(k01.x, pb, S[0]);
+        S[1] = fma(k01.y, pb, S[1]);
+        S[2] = fma(k23.x, pb, S[2]);
+        S[3] = fma(k23.y, pb, S[3]);
+      }
 #pragma unroll
-    for (int pol = 0; pol < 2; ++pol) {
-      const long long i = (2LL * a + pol) * p.N + tt;
-      const cpx u = shard_arg<STAGE>(p, i);
-      const cpx k = make_double2(-g * u.y, g * u.x);
-      if constexpr (STAGE == SH_PLAIN) {
-        p.Y[i] = k;
-      } else if constexpr (STAGE == SH_STAGE2) {
-        p.Z[i] = k;
-      } else if constexpr (STAGE == SH_STAGE3) {
-        const cpx x = p.X[i], y = p.Y[i], z = p.Z[i];
-        p.W[i] = cadd(x, k);
-        p.Z[i] = make_double2(x.x + sixth * y.x + third * z.x + third * k.x, x.y + sixth * y.y + third * z.y + third * k.y);
-      } else {
-        const cpx z = p.Z[i];
-        p.X[i] = make_double2(p.gain * fma(sixth, k.x, z.x), p.gain * fma(sixth, k.y, z.y));
+      for (int da = 0; da < 4; ++da) Ss[(a0 + da) * MMF_SH_T + lane] = p.hg * S[da];
+    }
+    __syncthreads();
+    if (!live) continue;
+    for (int r0 = warp; r0 < R; r0 += MMF_SH_WARPS * U) {
+      cpx x[U], y[U], z[U];   // stage 0: x = X; 1: x = X, y = Y; 2: x = X, y = Y, z = Z; 3: x = W, z = Z
+#pragma unroll
+      for (int j = 0; j < U; ++j) {
+        const int r = r0 + MMF_SH_WARPS * j;
+        if (r < R) {
+          const long long i = (long long)r * p.N + tt;
+          x[j] = (STAGE == SH_FINAL) ? p.W[i] : p.X[i];
+          if constexpr (STAGE == SH_STAGE2 || STAGE == SH_STAGE3) y[j] = p.Y[i];
+          if constexpr (STAGE == SH_STAGE3 || STAGE == SH_FINAL) z[j] = p.Z[i];
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < U; ++j) {
+        const int r = r0 + MMF_SH_WARPS * j;
+        if (r < R) {
+          const long long i = (long long)r * p.N + tt;
+          const double g = Ss[(r >> 1) * MMF_SH_T + lane];
+          cpx u = x[j];
+          if constexpr (STAGE == SH_STAGE2) u = make_double2(fma(0.5, y[j].x, x[j].x), fma(0.5, y[j].y, x[j].y));
+          if constexpr (STAGE == SH_STAGE3) u = make_double2(fma(0.5, z[j].x, x[j].x), fma(0.5, z[j].y, x[j].y));
+          const cpx k = make_double2(-g * u.y, g * u.x);
+          if constexpr (STAGE == SH_PLAIN) {
+            p.Y[i] = k;
+          } else if constexpr (STAGE == SH_STAGE2) {
+            p.Z[i] = k;
+          } else if constexpr (STAGE == SH_STAGE3) {
+            p.W[i] = cadd(x[j], k);
+            p.Z[i] = make_double2(x[j].x + sixth * y[j].x + third * z[j].x + third * k.x,
+                                  x[j].y + sixth * y[j].y + third * z[j].y + third * k.y);
+          } else {
+            p.X[i] = make_double2(p.gain * fma(sixth, k.x, z[j].x), p.gain * fma(sixth, k.y, z[j].y));
+          }
+        }
       }
     }
   }
