@@ -272,6 +272,20 @@ def run_probes(args):
             e["thread_inst_per_clk_per_sm"] = round(e.pop("thread_inst_per_s_per_sm") / clk, 1)
         else:
             e["clk_per_dmma_per_sm"] = round(clk / e.pop("warp_inst_per_s_per_sm"), 2)
+    # on-chip data paths of a 4096-point tile (16 complex values per thread): bytes per clock per SM where the kind moves
+    # a fixed 128 B per thread and operation, clock64 ticks per operation (per warp stage) otherwise
+    onchip = []
+    oc_names = ["tcgen05.ld 32x32b.x32 + wait", "tcgen05.st 32x32b.x32", "LDS.128 x 8", "SHFL.BFLY b32 x 32",
+                "tensor-memory trip, forward (st 32x32b, ld 16x256b)", "tensor-memory trip, reverse (st 16x256b, ld 32x32b)",
+                "warp-local exchange through shared memory", "group-wide exchange through shared memory (256 threads)",
+                "radix-16 stage, registers only", "radix-16 stage + 15 twiddles from shared memory"]
+    for kind, name in enumerate(oc_names):
+        for threads in ((256, 512) if kind == 7 else (32, 256, 512)):
+            ms, clk_op = binding.probe_onchip(kind, threads=threads, iters=2000)
+            e = {"kind": name, "threads_per_sm": threads, "clk_per_op": round(clk_op, 1)}
+            if kind < 4:
+                e["bytes_per_clk_per_sm"] = round(128.0 * threads / clk_op, 1)
+            onchip.append(e)
     R, N, N1, N2 = 240, 1 << 22, 1 << 10, 1 << 12
     buf = torch.zeros(R * N * 16, dtype=torch.uint8, device=dev)
     # (name, dim0 [doubles], dim1 [rows], stride [B], box0, box1, nbox, nct_log, c0_mul, c1_mul, ntiles, slots, bulk)
@@ -298,7 +312,7 @@ def run_probes(args):
         tma.append({"pattern": name, "tile_bytes": nbox * b0 * b1 * 8, "slots": slots, "ms": round(ms, 3),
                     "GB_s": round(by / (ms * 1e-3) / 1e9, 0), "GB_moved": round(by / 1e9, 1)})
     peak, src = load_peaks()
-    print(json.dumps({"probes": {"fp64": fp, "tma_copy": tma}, "sms": sms, "clocks_during_fp64": clocks,
+    print(json.dumps({"probes": {"fp64": fp, "onchip": onchip, "tma_copy": tma}, "sms": sms, "clocks_during_fp64": clocks,
                       "hbm_peak_GB_s": peak, "hbm_peak_source": src}), flush=True)
     return 0
 

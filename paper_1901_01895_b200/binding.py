@@ -20,7 +20,7 @@ SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_create_shard"
            "mmf_propagate_host", "mmf_propagate_host_batch", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
            "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_set_timing", "mmf_kernel_class_count",
            "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version",
-           "mmf_probe_fp64", "mmf_probe_tma_copy"]
+           "mmf_probe_fp64", "mmf_probe_tma_copy", "mmf_probe_onchip"]
 
 _lib = None
 
@@ -97,6 +97,8 @@ def lib():
     ull, u = ctypes.c_ulonglong, ctypes.c_uint
     L.mmf_probe_fp64.argtypes = [i, i, i, dp, dp]
     L.mmf_probe_fp64.restype = i
+    L.mmf_probe_onchip.argtypes = [i, i, i, dp, dp]
+    L.mmf_probe_onchip.restype = i
     L.mmf_probe_tma_copy.argtypes = [vp, sz, ull, ull, ull, u, u, i, i, i, i, ll, i, i, i, dp, dp]
     L.mmf_probe_tma_copy.restype = i
     L.mmf_version.argtypes = []
@@ -291,6 +293,14 @@ def probe_fp64(kind, threads=512, iters=4000):
     ms, n = ctypes.c_double(), ctypes.c_double()
     _check(lib().mmf_probe_fp64(int(kind), int(threads), int(iters), ctypes.byref(ms), ctypes.byref(n)), "mmf_probe_fp64")
     return ms.value, n.value
+
+
+def probe_onchip(kind, threads=512, iters=2000):
+    """mmf_probe_onchip: (ms per launch, clock64 ticks per operation with every warp of the CTA running the loop)."""
+    ms, clk = ctypes.c_double(), ctypes.c_double()
+    _check(lib().mmf_probe_onchip(int(kind), int(threads), int(iters), ctypes.byref(ms), ctypes.byref(clk)),
+           "mmf_probe_onchip")
+    return ms.value, clk.value
 
 
 def probe_tma_copy(buf, dim0, dim1, stride_bytes, box0, box1, nbox, nct_log, c0_mul, c1_mul, ntiles, slots=3, bulk=0,

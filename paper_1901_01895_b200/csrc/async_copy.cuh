@@ -131,16 +131,4 @@ __device__ __forceinline__ void tmem_words_to_c2(double2 (&e)[2], const int (&r)
   e[0] = make_double2(__hiloint2double(r[1], r[0]), __hiloint2double(r[3], r[2]));
   e[1] = make_double2(__hiloint2double(r[5], r[4]), __hiloint2double(r[7], r[6]));
 }
-// issue + wait in one
-__device__ __forceinline__ void tmem_ld_c2(double2 (&e)[2], uint32_t taddr) {
-  int r[8];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];\n"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-               : "r"(taddr));
-  asm volatile("tcgen05.wait::ld.sync.aligned;\n"
-               : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]));
-  e[0] = make_double2(__hiloint2double(r[1], r[0]), __hiloint2double(r[3], r[2]));
-  e[1] = make_double2(__hiloint2double(r[5], r[4]), __hiloint2double(r[7], r[6]));
-}
-
 }  // namespace mmf

@@ -374,9 +374,10 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
   cpx* tab = ring + ((size_t)S << MMF_TILE_LOG);
   uint64_t* full = reinterpret_cast<uint64_t*>(tab + ((TWN + 7) & ~7));
   uint64_t* done = full + S;
-  // The E values of a thread are the same for the 2 nbuf sub-tiles of an item: the first sub-tile takes them from
-  // global memory and parks them in tensor memory (64 columns of the thread's own lane), the others read them back
-  // from there — no global-load latency, no LSU traffic, no shared memory (none is left).
+  // The E values of a thread are the same for all sub-tiles of an item (polarisations x buffers): they are fetched
+  // into tensor memory (64 columns of the thread's own lane) at the top of the item's first tile — while no tile is
+  // held in registers, so all 16 loads are in flight at once — and every sub-tile reads them back from there: no
+  // global-load latency inside a transform, no LSU traffic, no shared memory (none is left).
   constexpr bool ECACHE = MODE == 0;
   // 4096-point transforms: the exchange between the last two stages goes through tensor memory (tmem_exchange.cuh),
   // 64 more columns per warp

@@ -7,6 +7,7 @@
 
 #include "../../include/mmf.h"
 #include "async_copy.cuh"
+#include "tmem_exchange.cuh"
 
 using namespace mmf;
 
@@ -143,6 +144,104 @@ int time_kernel(K launch, int reps, double* ms_out) {
   return MMF_OK;
 }
 
+// ---- on-chip data movement and stage arithmetic: what an exchange of a 4096-point tile costs each way ---------------
+// One CTA of `threads` threads per SM; every thread works on 16 complex values (the register tile of fft_core.cuh).
+// KIND 0: tcgen05.ld 32x32b.x32 + wait (128 B per thread)     1: tcgen05.st 32x32b.x32 (+ wait per four)
+// KIND 2: LDS.128 x 8 (128 B per thread)                      3: SHFL.BFLY b32 x 32 (128 B per thread)
+// KIND 4: tmem_trip_fwd   5: tmem_trip_rev   (tmem_exchange.cuh: a 2-bit lane <-> register exchange of the 16 values)
+// KIND 6: the warp-local exchange through shared memory (16 STS.128, warp barrier, 16 LDS.128, warp barrier)
+// KIND 7: the group-wide exchange (16 STS.128, group barrier, 16 LDS.128, group barrier; groups of 256 threads)
+// KIND 8: a radix-16 stage on registers only    9: a radix-16 stage with its 15 twiddles from a shared-memory table
+// clk_out: clock64 ticks per operation of the CTA's first thread (all warps run the same loop concurrently).
+template <int KIND>
+__global__ void __launch_bounds__(512, 1) k_probe_onchip(int iters, double* out, long long* clk) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  __shared__ uint32_t tw;
+  cpx* sbuf = reinterpret_cast<cpx*>(smem_raw);
+  if (threadIdx.x < 32) tmem_alloc(&tw, 512);
+  tmem_fence_before_sync();
+  for (int i = threadIdx.x; i < 2 * 4096; i += blockDim.x) sbuf[i] = make_double2(0.6, 0.8);
+  __syncthreads();
+  tmem_fence_after_sync();
+  const uint32_t warp = threadIdx.x >> 5;
+  const uint32_t xa = tw + (((warp & 3) * 32) << 16) + (warp >> 2) * 128;
+  const int grp = threadIdx.x >> 8, t = threadIdx.x & 255;
+  cpx* s = sbuf + ((size_t)grp << 12);
+  const Tm12 L = tm12_layout(t);
+  cpx v[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) v[j] = make_double2(1e-3 * (threadIdx.x + j), 1e-3 * j);
+  int w[32];
+#pragma unroll
+  for (int j = 0; j < 32; ++j) w[j] = threadIdx.x + j;
+  const long long t0 = clock64();
+  for (int it = 0; it < iters; ++it) {
+    if constexpr (KIND == 0) {
+      int q[32];
+      tmem_ld_32x32b_x32(q, xa + 32 * (it & 3));
+      tmem_wait_ld32(q);
+#pragma unroll
+      for (int j = 0; j < 32; ++j) w[j] ^= q[j];   // every loaded word is consumed
+    } else if constexpr (KIND == 1) {
+      tmem_st_32x32b_x32(xa + 32 * (it & 3), w);
+      if ((it & 3) == 3) tmem_wait_st();
+      w[0] += it;
+    } else if constexpr (KIND == 2) {
+      const uint4* q = reinterpret_cast<const uint4*>(smem_raw);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const uint4 x = q[(threadIdx.x + 512 * j + 37 * (it & 3) + (w[0] & 1)) & 8191];
+        w[0] += x.x;
+      }
+    } else if constexpr (KIND == 3) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) w[j] = __shfl_xor_sync(0xffffffffu, w[j], 1 + (j & 15));
+    } else if constexpr (KIND == 4) {
+      tmem_trip_fwd(v, xa);
+    } else if constexpr (KIND == 5) {
+      tmem_trip_rev(v, xa);
+    } else if constexpr (KIND == 6) {
+      tile_sts<4>(v, s, stage_base<4>(t));
+      __syncwarp();
+      tile_lds<0>(v, s, stage_base<0>(t));
+      __syncwarp();
+    } else if constexpr (KIND == 7) {
+      tile_sts12<8>(v, s, L.base1);
+      group_barrier(1 + grp, MMF_GROUP_THREADS);
+      tile_lds12<4>(v, s, L.base2);
+      group_barrier(1 + grp, MMF_GROUP_THREADS);
+    } else if constexpr (KIND == 8) {
+      stage_math<12, 0, 0, 4, +1, true>(v, 0, sbuf);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) { v[j].x *= 0.25; v[j].y *= 0.25; }
+    } else {
+      stage_math<12, 0, 4, 4, +1, true>(v, t & 15, sbuf);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) { v[j].x *= 0.25; v[j].y *= 0.25; }
+    }
+    if constexpr (KIND >= 4 && KIND <= 7) v[0].x += 1.0;
+  }
+  const long long t1 = clock64();
+  double acc = 0;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) acc += v[j].x + v[j].y;
+#pragma unroll
+  for (int j = 0; j < 32; ++j) acc += w[j];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+  if (threadIdx.x == 0 && blockIdx.x == 0) clk[0] = t1 - t0;
+  tmem_fence_before_sync();
+  __syncthreads();
+  if (threadIdx.x < 32) tmem_dealloc(tw, 512);
+}
+
+template <int KIND>
+int run_onchip(int sms, int threads, int iters, double* out, long long* clk, double* ms_out) {
+  const size_t smem = 2 * 4096 * sizeof(cpx);
+  if (cudaFuncSetAttribute(k_probe_onchip<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return MMF_ECUDA;
+  return time_kernel([&] { k_probe_onchip<KIND><<<sms, threads, smem>>>(iters, out, clk); }, 1, ms_out);
+}
+
 }  // namespace
 
 extern "C" {
@@ -211,6 +310,32 @@ int mmf_probe_tma_copy(void* buf_dev, size_t buf_bytes, unsigned long long dim0,
   const long long grid = ntiles < sms ? ntiles : sms;
   const int rc = time_kernel([&] { k_probe_copy<<<(unsigned)grid, 32, smem>>>(map, p, (char*)buf_dev); }, reps, ms_out);
   *bytes_out = 2.0 * (double)ntiles * (double)slot_bytes;  // read + write
+  return rc;
+}
+
+int mmf_probe_onchip(int kind, int threads, int iters, double* ms_out, double* clk_per_op_out) {
+  if (!ms_out || !clk_per_op_out || iters < 1 || kind < 0 || kind > 9) return MMF_EINVAL;
+  if (threads < 32 || threads > 512 || (threads & 31) || (kind == 7 && (threads & 255))) return MMF_EINVAL;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return MMF_ECUDA;
+  double* out = nullptr;
+  long long* clk = nullptr;
+  if (cudaMalloc((void**)&out, sizeof(double) * 512 * (size_t)sms) != cudaSuccess) return MMF_ENOMEM;
+  if (cudaMalloc((void**)&clk, sizeof(long long)) != cudaSuccess) { cudaFree(out); return MMF_ENOMEM; }
+  int rc = MMF_EINVAL;
+  switch (kind) {
+#define MMF_ONCHIP_CASE(K) case K: rc = run_onchip<K>(sms, threads, iters, out, clk, ms_out); break;
+    MMF_ONCHIP_CASE(0) MMF_ONCHIP_CASE(1) MMF_ONCHIP_CASE(2) MMF_ONCHIP_CASE(3) MMF_ONCHIP_CASE(4) MMF_ONCHIP_CASE(5)
+    MMF_ONCHIP_CASE(6) MMF_ONCHIP_CASE(7) MMF_ONCHIP_CASE(8) MMF_ONCHIP_CASE(9)
+#undef MMF_ONCHIP_CASE
+    default: break;
+  }
+  long long h = 0;
+  if (rc == MMF_OK && cudaMemcpy(&h, clk, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) rc = MMF_ECUDA;
+  cudaFree(out);
+  cudaFree(clk);
+  *clk_per_op_out = (double)h / iters;
   return rc;
 }
 

@@ -1,12 +1,13 @@
 // tmem_exchange.cuh — the warp-local exchange of a 4096-point transform through TENSOR MEMORY instead of shared memory.
 //
-// Why.  Pass B (k_rows, fft_kernels.cuh) is bound by its shared-memory traffic: five exchanges of 16 B each way per
-// point at 128 B per clock per SM (profiles/r2a_ncu_full_cfg4.md: LSU data pipe 71 %).  Tensor memory moves
-// ~1.6 KB per clock per SM on the tcgen05.ld / tcgen05.st path (measured: 3.1 / 1.7 TB/s per SM against 0.22 for
-// LDS.128), on a datapath of its own, but a thread only reaches its own lane with the 32x32b shape.  The 16x256b shape
-// is the exception: thread T of a warp reads (writes) lanes 8 q + (T >> 2) (+ 16 h for the second instruction) and,
-// of every group of four 64-bit columns, column (T & 3).  A store with one shape followed by a load with the other
-// therefore MOVES data between the lanes of a warp:
+// Why.  Pass B (k_rows, fft_kernels.cuh) keeps its shared-memory pipe busy 71 % of the time with five exchanges of 16 B
+// each way per point at 128 B per clock per SM (profiles/r2a_ncu_full_cfg4.md).  Tensor memory is a second on-chip
+// store with a datapath of its own (bench.py --probes, profiles/r2b_probes.json: tcgen05.st 32x32b moves 840 B per clock
+// per SM, tcgen05.ld at least 330, against 114-128 for LDS.128 and SHFL), but with that shape a thread only reaches its
+// own lane.  The 16x256b shape is the
+// exception: thread T of a warp reads (writes) lanes 8 q + (T >> 2) (+ 16 h for the second instruction) and, of every
+// group of four 64-bit columns, column (T & 3) (layout determined with a probe kernel).  A store with one shape
+// followed by a load with the other therefore MOVES data between the lanes of a warp:
 //   store 32x32b (thread L writes doubles d = 0..15 of its lane), load 16x256b:
 //       thread T receives, as value (h, q, g), what thread L = 16 h + 8 q + (T >> 2) wrote as double 4 g + (T & 3).
 //   In index bits: the two top lane bits of the writer become register bits, the two low register bits of the writer
