@@ -349,7 +349,8 @@ def run_mmf(args):
         assert args.method == "rk4ip" and not general, "--shard: rk4ip with the Manakov kappa"
         mode0, m, beta_l, kappa_rows = sharded.shard_arguments(p.beta, p.kappa, rank, world)
         H = H[2 * mode0:2 * (mode0 + m)]
-        shard = sharded.CudaShardStages(p.M, mode0, p.N, p.dt, p.h, p.alpha, beta_l, p.gamma, kappa_rows, device=dev)
+        shard = sharded.CudaShardStages(p.M, mode0, p.N, p.dt, p.h, p.alpha, beta_l, p.gamma, kappa_rows, device=dev,
+                                        chunks=args.shard_chunks)
     X = torch.empty(tuple(H.shape), dtype=torch.complex128, device=dev)
     X.copy_(H)
     if world > 1 and shard is None:                  # replicas: a launch-power sweep, one power per rank
@@ -369,7 +370,8 @@ def run_mmf(args):
                "agrawal": lambda X_, n_: plan.propagate_ssfm_agrawal(X_, n_, niter=args.niter)}[args.method]
     if shard is not None:
         def advance(X_, n_):
-            sharded.propagate(shard, X_, n_, lambda: sharded.all_gather_rows(shard.P_all, shard.mode0, shard.M_local, dist))
+            sharded.propagate(shard, X_, n_, lambda c: sharded.all_gather_rows(shard.P_all[c], shard.mode0, shard.M_local, dist,
+                                                                             async_op=world > 1))
     advance(X, args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
@@ -589,6 +591,8 @@ def main():
     ap.add_argument("--shard", action="store_true",
                     help="row-sharded path (SURVEY.md NEXT-3): every rank propagates M / world modes and all-gathers the mode "
                          "powers; with one GPU it measures the split kernels alone")
+    ap.add_argument("--shard-chunks", type=int, default=1,
+                    help="--shard: time chunks per evaluation of N (the gather of one chunk overlaps the kernels of the next)")
     ap.add_argument("--modes", type=int, default=None, help="override the config's mode count M (extra data points)")
     ap.add_argument("--logn", type=int, default=None, help="override the config's N = 2^logn (extra data points)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

@@ -125,16 +125,19 @@ int mmf_propagate_host_batch(mmf_plan *plan, void *const *A_hosts, int nfields, 
  *              powers(3); all-gather; apply(3, gain)   A <- gain (D(bracket) + h N(u4) u4 / 6)   (6e), (6f)
  *              powers(0); all-gather; apply(0) for the next step (not after the last one)
  *   mmf_shard_end()                            the result is in A
- * mmf_shard_powers writes rows mode0 .. mode0 + M_local - 1 of P_all (device, [M_total][N] doubles, row-major):
- *   P_all[b][t] = |u_bx(t)|^2 + |u_by(t)|^2, u the argument of the stage's N; the caller's all-gather fills the other
- *   rows; mmf_shard_apply reads all of them.  For N > 4096 the sample index t of P_all is the library's internal
- *   (blocked) order — the same on every rank, since it depends on N only.  stage: 0..3 as listed.
+ * mmf_shard_powers / mmf_shard_apply work on a TIME CHUNK: samples t_first .. t_first + t_count - 1 (the whole axis:
+ *   0, N), with P_dev (device, [M_total][t_count] doubles, row-major) the chunk's own power block.  powers writes rows
+ *   mode0 .. mode0 + M_local - 1: P[b][t - t_first] = |u_bx(t)|^2 + |u_by(t)|^2, u the argument of the stage's N; the
+ *   caller's all-gather fills the other rows; apply reads all of them.  Chunks let the gather of one chunk overlap
+ *   the kernels of its neighbours.  For N > 4096 the sample index is the library's internal (blocked)
+ *   order — the same on every rank, since it depends on N only.  stage: 0..3 as listed.
  * Shard plans accept only the mmf_shard_* calls, mmf_apply_linear and the timing / debug calls. */
 int mmf_plan_create_shard(mmf_plan **out, int M_local, int M_total, int mode0, long long N, double dt, double h,
                           double alpha, const double *beta, int K, double gamma, const double *kappa_rows);
 int mmf_shard_begin(mmf_plan *plan, void *A_dev, void *cuda_stream);
-int mmf_shard_powers(mmf_plan *plan, int stage, void *P_all_dev, void *cuda_stream);
-int mmf_shard_apply(mmf_plan *plan, int stage, const void *P_all_dev, double gain, void *cuda_stream);
+int mmf_shard_powers(mmf_plan *plan, int stage, void *P_dev, long long t_first, long long t_count, void *cuda_stream);
+int mmf_shard_apply(mmf_plan *plan, int stage, const void *P_dev, long long t_first, long long t_count, double gain,
+                    void *cuda_stream);
 int mmf_shard_linear(mmf_plan *plan, int which, void *cuda_stream);
 int mmf_shard_end(mmf_plan *plan, void *cuda_stream);
 

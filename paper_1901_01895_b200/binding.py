@@ -48,9 +48,9 @@ def lib():
     L.mmf_plan_create_shard.restype = i
     L.mmf_shard_begin.argtypes = [vp, vp, vp]
     L.mmf_shard_begin.restype = i
-    L.mmf_shard_powers.argtypes = [vp, i, vp, vp]
+    L.mmf_shard_powers.argtypes = [vp, i, vp, ll, ll, vp]
     L.mmf_shard_powers.restype = i
-    L.mmf_shard_apply.argtypes = [vp, i, vp, d, vp]
+    L.mmf_shard_apply.argtypes = [vp, i, vp, ll, ll, d, vp]
     L.mmf_shard_apply.restype = i
     L.mmf_shard_linear.argtypes = [vp, i, vp]
     L.mmf_shard_linear.restype = i
@@ -185,18 +185,21 @@ class Plan:
     def shard_begin(self, A, stream=None):
         _check(lib().mmf_shard_begin(self._h, self._field_ptr(A), _stream_ptr(stream)), "mmf_shard_begin")
 
-    def shard_powers(self, stage, P_all, stream=None):
+    def _chunk_ptr(self, P, t_count):
         import torch
-        assert P_all.is_cuda and P_all.dtype == torch.float64 and P_all.is_contiguous()
-        assert tuple(P_all.shape) == (self.M_total, self.N)
-        _check(lib().mmf_shard_powers(self._h, int(stage), ctypes.c_void_p(P_all.data_ptr()), _stream_ptr(stream)),
-               "mmf_shard_powers")
+        assert P.is_cuda and P.dtype == torch.float64 and P.is_contiguous()
+        assert tuple(P.shape) == (self.M_total, t_count), (tuple(P.shape), self.M_total, t_count)
+        return ctypes.c_void_p(P.data_ptr())
 
-    def shard_apply(self, stage, P_all, gain=1.0, stream=None):
-        import torch
-        assert P_all.is_cuda and P_all.dtype == torch.float64 and P_all.is_contiguous()
-        assert tuple(P_all.shape) == (self.M_total, self.N)
-        _check(lib().mmf_shard_apply(self._h, int(stage), ctypes.c_void_p(P_all.data_ptr()), float(gain),
+    def shard_powers(self, stage, P, t_first=0, t_count=None, stream=None):
+        """P: CUDA float64 [M_total][t_count], the power block of samples t_first .. t_first + t_count - 1."""
+        t_count = self.N if t_count is None else int(t_count)
+        _check(lib().mmf_shard_powers(self._h, int(stage), self._chunk_ptr(P, t_count), int(t_first), t_count,
+                                      _stream_ptr(stream)), "mmf_shard_powers")
+
+    def shard_apply(self, stage, P, t_first=0, t_count=None, gain=1.0, stream=None):
+        t_count = self.N if t_count is None else int(t_count)
+        _check(lib().mmf_shard_apply(self._h, int(stage), self._chunk_ptr(P, t_count), int(t_first), t_count, float(gain),
                                      _stream_ptr(stream)), "mmf_shard_apply")
 
     def shard_linear(self, which, stream=None):

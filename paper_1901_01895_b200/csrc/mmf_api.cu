@@ -648,15 +648,17 @@ void free_tables(mmf_plan* p) {
 
 namespace {
 template <int STAGE>
-int launch_shard(mmf_plan* p, bool pow, double* P_all, double gain, cudaStream_t st) {
+int launch_shard(mmf_plan* p, bool pow, double* P_all, long long t_first, long long t_count, double gain, cudaStream_t st) {
   ShardParams q;
   q.X = p->shard_X; q.Y = p->Y; q.Z = p->Z; q.W = p->W;
   q.kappa_rows = p->d_kappa; q.P_all = P_all;
   q.hg = p->h * p->gamma; q.gain = gain;
   q.M_local = p->M; q.M_total = p->M_total; q.mode0 = p->mode0; q.N = p->N;
-  const unsigned grid = (unsigned)((p->N + MMF_SH_T - 1) / MMF_SH_T);
+  q.t_first = t_first; q.t_count = t_count;
+  const double frac = (double)t_count / (double)p->N;   // of the launch's full-axis traffic
+  const unsigned grid = (unsigned)((t_count + MMF_SH_T - 1) / MMF_SH_T);
   if (pow) {
-    LaunchTimer lt(p, KC_SHARD_POW, STAGE == SH_PLAIN || STAGE == SH_FINAL ? 1.0 : 2.0, st);
+    LaunchTimer lt(p, KC_SHARD_POW, frac * (STAGE == SH_PLAIN || STAGE == SH_FINAL ? 1.0 : 2.0), st);
     CU(launch_kernel(p, k_shard_pow<STAGE>, grid, MMF_SH_T * MMF_SH_WARPS, 0, st, q));
   } else {
     const size_t smem = shard_apply_smem_bytes(p->M, p->M_total);
@@ -669,18 +671,20 @@ int launch_shard(mmf_plan* p, bool pow, double* P_all, double gain, cudaStream_t
     if (occ < 1) return MMF_EINVAL;
     unsigned pgrid = (unsigned)(p->num_sms * occ);   // persistent: kappa goes to shared memory once per CTA
     if (pgrid > grid) pgrid = grid;
-    LaunchTimer lt(p, KC_SHARD_APPLY, STAGE == SH_PLAIN ? 2 : STAGE == SH_STAGE2 ? 3 : STAGE == SH_STAGE3 ? 5 : 3, st);
+    LaunchTimer lt(p, KC_SHARD_APPLY, frac * (STAGE == SH_PLAIN ? 2 : STAGE == SH_STAGE2 ? 3 : STAGE == SH_STAGE3 ? 5 : 3), st);
     CU(launch_kernel(p, kern, pgrid, MMF_SH_T * MMF_SH_WARPS, smem, st, q));
   }
   p->launches++;
   return MMF_OK;
 }
-int shard_stage(mmf_plan* p, int stage, bool pow, double* P_all, double gain, cudaStream_t st) {
+int shard_stage(mmf_plan* p, int stage, bool pow, double* P_all, long long t_first, long long t_count, double gain,
+                cudaStream_t st) {
+  if (t_first < 0 || t_count < 1 || t_first + t_count > p->N) return MMF_EINVAL;
   switch (stage) {
-    case SH_PLAIN: return launch_shard<SH_PLAIN>(p, pow, P_all, gain, st);
-    case SH_STAGE2: return launch_shard<SH_STAGE2>(p, pow, P_all, gain, st);
-    case SH_STAGE3: return launch_shard<SH_STAGE3>(p, pow, P_all, gain, st);
-    case SH_FINAL: return launch_shard<SH_FINAL>(p, pow, P_all, gain, st);
+    case SH_PLAIN: return launch_shard<SH_PLAIN>(p, pow, P_all, t_first, t_count, gain, st);
+    case SH_STAGE2: return launch_shard<SH_STAGE2>(p, pow, P_all, t_first, t_count, gain, st);
+    case SH_STAGE3: return launch_shard<SH_STAGE3>(p, pow, P_all, t_first, t_count, gain, st);
+    case SH_FINAL: return launch_shard<SH_FINAL>(p, pow, P_all, t_first, t_count, gain, st);
     default: return MMF_EINVAL;
   }
 }
@@ -1204,14 +1208,15 @@ int mmf_shard_begin(mmf_plan* p, void* A_dev, void* cuda_stream) {
   return MMF_OK;
 }
 
-int mmf_shard_powers(mmf_plan* p, int stage, void* P_all_dev, void* cuda_stream) {
-  if (!shard_ready(p) || !p->shard_A || !P_all_dev || ((size_t)P_all_dev & 7) != 0) return MMF_EINVAL;
-  return shard_stage(p, stage, true, (double*)P_all_dev, 1.0, (cudaStream_t)cuda_stream);
+int mmf_shard_powers(mmf_plan* p, int stage, void* P_dev, long long t_first, long long t_count, void* cuda_stream) {
+  if (!shard_ready(p) || !p->shard_A || !P_dev || ((size_t)P_dev & 7) != 0) return MMF_EINVAL;
+  return shard_stage(p, stage, true, (double*)P_dev, t_first, t_count, 1.0, (cudaStream_t)cuda_stream);
 }
 
-int mmf_shard_apply(mmf_plan* p, int stage, const void* P_all_dev, double gain, void* cuda_stream) {
-  if (!shard_ready(p) || !p->shard_A || !P_all_dev || ((size_t)P_all_dev & 7) != 0 || !std::isfinite(gain)) return MMF_EINVAL;
-  return shard_stage(p, stage, false, (double*)P_all_dev, gain, (cudaStream_t)cuda_stream);
+int mmf_shard_apply(mmf_plan* p, int stage, const void* P_dev, long long t_first, long long t_count, double gain,
+                    void* cuda_stream) {
+  if (!shard_ready(p) || !p->shard_A || !P_dev || ((size_t)P_dev & 7) != 0 || !std::isfinite(gain)) return MMF_EINVAL;
+  return shard_stage(p, stage, false, (double*)P_dev, t_first, t_count, gain, (cudaStream_t)cuda_stream);
 }
 
 int mmf_shard_linear(mmf_plan* p, int which, void* cuda_stream) {

@@ -4,6 +4,9 @@
 //
 // A rank owns M_local spatial modes (2 M_local rows) of a fibre with M_total modes, modes mode0 .. mode0 + M_local - 1.
 // One evaluation of N = i h gamma (sum_b kappa_ab P_b) is two kernels with a collective between them:
+// Both kernels work on a TIME CHUNK [t_first, t_first + t_count) with its own contiguous [M_total][t_count] power block, so
+// that the all-gather of one chunk overlaps the kernels of its neighbours (the B200 form of the paper's overlap of
+// calc_nonlinear_own with the transfers; sharded.py pipelines them).
 //   k_shard_pow<STAGE>     P_all[mode0 + a][t] = |u_ax(t)|^2 + |u_ay(t)|^2   for the rank's own modes (real, PAPER.md:111:
 //                          "stored real to halve the traffic"), u the argument of the stage's N;
 //   (all-gather of the M_total x N real matrix P_all: torch.distributed / NCCL, driven by sharded.py)
@@ -29,10 +32,11 @@ struct ShardParams {
   cpx* Z;
   cpx* W;
   const double* __restrict__ kappa_rows;  // [M_local][M_total]
-  double* P_all;                          // [M_total][N]
+  double* P_all;                          // [M_total][t_count]: the powers of samples t_first .. t_first + t_count - 1
   double hg, gain;
   int M_local, M_total, mode0;
   long long N;
+  long long t_first, t_count;             // the time chunk this launch works on (the whole axis: 0, N)
 };
 
 #define MMF_SH_T 32
@@ -53,17 +57,18 @@ __device__ __forceinline__ cpx shard_arg(const ShardParams& p, long long i) {
   }
 }
 
-// grid = ceil(N / 32), block = 512
+// grid = ceil(t_count / 32), block = 512
 template <int STAGE>
 __global__ void __launch_bounds__(MMF_SH_T* MMF_SH_WARPS) k_shard_pow(ShardParams p) {
   pdl_launch_dependents();
   pdl_wait();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long long tt = (long long)blockIdx.x * MMF_SH_T + lane;
-  if (tt >= p.N) return;
+  const long long tc = (long long)blockIdx.x * MMF_SH_T + lane;   // sample inside the chunk
+  if (tc >= p.t_count) return;
+  const long long tt = p.t_first + tc;
   for (int a = warp; a < p.M_local; a += MMF_SH_WARPS) {
     const cpx ux = shard_arg<STAGE>(p, (2LL * a) * p.N + tt), uy = shard_arg<STAGE>(p, (2LL * a + 1) * p.N + tt);
-    p.P_all[(long long)(p.mode0 + a) * p.N + tt] = (ux.x * ux.x + ux.y * ux.y) + (uy.x * uy.x + uy.y * uy.y);
+    p.P_all[(long long)(p.mode0 + a) * p.t_count + tc] = (ux.x * ux.x + ux.y * ux.y) + (uy.x * uy.x + uy.y * uy.y);
   }
 }
 
@@ -97,12 +102,13 @@ __global__ void __launch_bounds__(MMF_SH_T* MMF_SH_WARPS) k_shard_apply(ShardPar
   const double third = 1.0 / 3.0, sixth = 1.0 / 6.0;
   const int R = 2 * p.M_local;
   constexpr int U = 4;   // field rows per warp and batch in phase 3
-  const long long ntile = (p.N + MMF_SH_T - 1) / MMF_SH_T;
+  const long long ntile = (p.t_count + MMF_SH_T - 1) / MMF_SH_T;
   for (long long tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
-    const long long tt = tile * MMF_SH_T + lane;
-    const bool live = tt < p.N;
+    const long long tc = tile * MMF_SH_T + lane;   // sample inside the chunk
+    const long long tt = p.t_first + tc;
+    const bool live = tc < p.t_count;
     __syncthreads();   // the previous tile's P and S are no longer read (and, first time round, ks is complete)
-    for (int b = warp; b < p.M_total; b += MMF_SH_WARPS) P[b * MMF_SH_T + lane] = live ? p.P_all[(long long)b * p.N + tt] : 0.0;
+    for (int b = warp; b < p.M_total; b += MMF_SH_WARPS) P[b * MMF_SH_T + lane] = live ? p.P_all[(long long)b * p.t_count + tc] : 0.0;
     __syncthreads();
     for (int a0 = 4 * warp; a0 < p.M_local; a0 += 4 * MMF_SH_WARPS) {
       double S[4] = {0.0, 0.0, 0.0, 0.0};

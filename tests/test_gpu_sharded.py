@@ -10,29 +10,29 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 
-def _run_shards(p, A, steps, world, span=0, gain=1.0):
+def _run_shards(p, A, steps, world, span=0, gain=1.0, chunks=1):
     import torch
     from paper_1901_01895_b200 import sharded
     stages, fields, rng = [], [], []
     for r in range(world):
         mode0, m, beta_l, kappa_rows = sharded.shard_arguments(p.beta, p.kappa, r, world)
-        stages.append(sharded.CudaShardStages(p.M, mode0, p.N, p.dt, p.h, p.alpha, beta_l, p.gamma, kappa_rows))
+        stages.append(sharded.CudaShardStages(p.M, mode0, p.N, p.dt, p.h, p.alpha, beta_l, p.gamma, kappa_rows, chunks=chunks))
         fields.append(torch.from_numpy(np.ascontiguousarray(A[2 * mode0:2 * (mode0 + m)])).cuda())
         rng.append((mode0, m))
     bar = threading.Barrier(world)
     errs = []
 
-    def gather(r):
+    def gather(r, c):
         bar.wait()                      # every rank has enqueued its powers kernel (same stream: ordered)
         for j, (m0, m) in enumerate(rng):
             if j != r:
-                stages[r].P_all[m0:m0 + m].copy_(stages[j].P_all[m0:m0 + m])
+                stages[r].P_all[c, m0:m0 + m].copy_(stages[j].P_all[c, m0:m0 + m])
         bar.wait()                      # nobody overwrites its rows before everybody has copied them
 
     def rank(r):
         try:
             torch.cuda.set_device(0)
-            sharded.propagate(stages[r], fields[r], steps, lambda: gather(r), span=span, gain=gain)
+            sharded.propagate(stages[r], fields[r], steps, lambda c: gather(r, c), span=span, gain=gain)
         except Exception as e:          # pragma: no cover
             errs.append(e)
             bar.abort()
@@ -50,14 +50,15 @@ def _run_shards(p, A, steps, world, span=0, gain=1.0):
     return np.concatenate([f.cpu().numpy() for f in fields], axis=0), launches
 
 
-@pytest.mark.parametrize("cfg,M,logn,steps,world", [(0, 2, 12, 5, 1), (0, 2, 12, 5, 2), (1, 6, 14, 3, 1), (1, 6, 14, 3, 2),
-                                                   (1, 6, 14, 3, 3), (4, 4, 16, 2, 4), (2, 12, 8, 3, 4)])
-def test_sharded_propagation_matches_oracle(cfg, M, logn, steps, world):
+@pytest.mark.parametrize("cfg,M,logn,steps,world,chunks", [(0, 2, 12, 5, 1, 1), (0, 2, 12, 5, 2, 2), (1, 6, 14, 3, 1, 4),
+                                                          (1, 6, 14, 3, 2, 1), (1, 6, 14, 3, 3, 8), (4, 4, 16, 2, 4, 2),
+                                                          (2, 12, 8, 3, 4, 1), (2, 12, 8, 3, 4, 8)])
+def test_sharded_propagation_matches_oracle(cfg, M, logn, steps, world, chunks):
     from oracle import oracle
     from paper_1901_01895_b200 import workloads
     p = workloads.problem(cfg, M=M, N=1 << logn, steps=steps)
     A = p.field() * (8.0 if cfg < 4 else 1.0)
-    got, launches = _run_shards(p, A, steps, world)
+    got, launches = _run_shards(p, A, steps, world, chunks=chunks)
     want = oracle.rk4ip(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, steps)
     err = workloads.rel_l2_per_field(got, want)
     assert err.max() <= 1e-10, err
@@ -91,7 +92,7 @@ def test_powers_integer_exact_and_offsets():
     st.begin(X)
     st.powers(sharded.SH_PLAIN)
     st.end()
-    P = st.P_all.cpu().numpy()
+    P = st.P_all[0].cpu().numpy()
     sq = A.real ** 2 + A.imag ** 2                      # exact in fp64 for these integers
     want = sq[0::2] + sq[1::2]
     assert np.array_equal(P[mode0:mode0 + m], want[mode0:mode0 + m])

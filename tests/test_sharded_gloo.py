@@ -16,7 +16,7 @@ from paper_1901_01895_b200 import sharded, workloads
 class OracleShardStages:
     """begin / powers / apply / linear / end of sharded.propagate on numpy arrays, from Eq. (1) and Eq. (6)."""
 
-    def __init__(self, M_total, mode0, N, dt, h, alpha, beta_local, gamma, kappa_rows):
+    def __init__(self, M_total, mode0, N, dt, h, alpha, beta_local, gamma, kappa_rows, chunks=1):
         import torch
         from oracle import oracle
         self.orc = oracle
@@ -24,7 +24,8 @@ class OracleShardStages:
         self.hg = h * gamma
         self.kappa_rows = np.asarray(kappa_rows)
         self.E = oracle.linear_table(self.m, N, dt, 0.5 * h, alpha, beta_local)
-        self.P_all = torch.zeros((M_total, N), dtype=torch.float64)
+        self.ranges = sharded.chunk_ranges(N, chunks)
+        self.P_all = torch.zeros((chunks, M_total, N // chunks), dtype=torch.float64)
 
     def begin(self, A):
         self.X = A
@@ -32,27 +33,29 @@ class OracleShardStages:
         self.Z = np.zeros_like(A)
         self.W = np.zeros_like(A)
 
-    def _arg(self, stage):
-        return (self.X, self.X + 0.5 * self.Y, self.X + 0.5 * self.Z, self.W)[stage]
+    def _arg(self, stage, sl):
+        return (self.X[:, sl], self.X[:, sl] + 0.5 * self.Y[:, sl], self.X[:, sl] + 0.5 * self.Z[:, sl], self.W[:, sl])[stage]
 
-    def powers(self, stage):
-        u = self._arg(stage)
-        P = (np.abs(u[0::2]) ** 2 + np.abs(u[1::2]) ** 2)
-        self.P_all.numpy()[self.mode0:self.mode0 + self.m] = P
+    def powers(self, stage, c=0):
+        t0, n = self.ranges[c]
+        u = self._arg(stage, slice(t0, t0 + n))
+        self.P_all[c].numpy()[self.mode0:self.mode0 + self.m] = np.abs(u[0::2]) ** 2 + np.abs(u[1::2]) ** 2
 
-    def apply(self, stage, gain=1.0):
-        u = self._arg(stage)
-        S = self.kappa_rows @ self.P_all.numpy()                     # [m][N]
+    def apply(self, stage, c=0, gain=1.0):
+        t0, n = self.ranges[c]
+        sl = slice(t0, t0 + n)
+        u = self._arg(stage, sl)
+        S = self.kappa_rows @ self.P_all[c].numpy()                  # [m][n]
         k = 1j * self.hg * np.repeat(S, 2, axis=0) * u
         if stage == 0:
-            self.Y[:] = k
+            self.Y[:, sl] = k
         elif stage == 1:
-            self.Z[:] = k
+            self.Z[:, sl] = k
         elif stage == 2:
-            self.W[:] = self.X + k
-            self.Z[:] = self.X + self.Y / 6 + self.Z / 3 + k / 3
+            self.W[:, sl] = self.X[:, sl] + k
+            self.Z[:, sl] = self.X[:, sl] + self.Y[:, sl] / 6 + self.Z[:, sl] / 3 + k / 3
         else:
-            self.X[:] = gain * (self.Z + k / 6)
+            self.X[:, sl] = gain * (self.Z[:, sl] + k / 6)
 
     def linear(self, which):
         for buf in ((self.X, self.Y) if which == 0 else (self.W, self.Z)):
@@ -68,7 +71,7 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _worker(rank, world, port, out, M, N, steps):
+def _worker(rank, world, port, out, M, N, steps, chunks):
     import torch.distributed as dist
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group(backend="gloo", rank=rank, world_size=world)
@@ -76,15 +79,18 @@ def _worker(rank, world, port, out, M, N, steps):
         p = workloads.problem(0, M=M, N=N, steps=steps)
         A = p.field() * 30.0                                   # strong enough for the nonlinear term to matter
         mode0, m, beta_l, kappa_rows = sharded.shard_arguments(p.beta, p.kappa, rank, world)
-        st = OracleShardStages(p.M, mode0, p.N, p.dt, p.h, p.alpha, beta_l, p.gamma, kappa_rows)
+        st = OracleShardStages(p.M, mode0, p.N, p.dt, p.h, p.alpha, beta_l, p.gamma, kappa_rows, chunks=chunks)
         mine = np.ascontiguousarray(A[2 * mode0:2 * (mode0 + m)])
-        sharded.propagate(st, mine, steps, lambda: sharded.all_gather_rows(st.P_all, mode0, m, dist), span=2, gain=1.01)
+        # chunks > 1: asynchronous gathers, waited for chunk by chunk (the pipelined form the GPU path runs)
+        sharded.propagate(st, mine, steps, lambda c: sharded.all_gather_rows(st.P_all[c], mode0, m, dist, async_op=chunks > 1),
+                          span=2, gain=1.01)
         out.put((rank, mode0, m, mine))
     finally:
         dist.destroy_process_group()
 
 
-def test_two_ranks_reproduce_the_unsharded_oracle():
+@pytest.mark.parametrize("chunks", [1, 4])
+def test_two_ranks_reproduce_the_unsharded_oracle(chunks):
     import torch.multiprocessing as mp
     from oracle import oracle
     oracle.build()
@@ -92,7 +98,7 @@ def test_two_ranks_reproduce_the_unsharded_oracle():
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, out, M, N, steps)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, out, M, N, steps, chunks)) for r in range(2)]
     for pr in procs:
         pr.start()
     res = sorted((out.get(timeout=180) for _ in procs), key=lambda t: t[0])
@@ -126,5 +132,8 @@ def test_single_process_gather_is_a_no_op():
     import torch
     P = torch.arange(12.0, dtype=torch.float64).reshape(4, 3)
     Q = P.clone()
-    sharded.all_gather_rows(P, 0, 4, None)
+    assert sharded.all_gather_rows(P, 0, 4, None) is None
     assert torch.equal(P, Q)
+    assert sharded.chunk_ranges(256, 4) == [(0, 64), (64, 64), (128, 64), (192, 64)]
+    with pytest.raises(ValueError):
+        sharded.chunk_ranges(256, 16)
