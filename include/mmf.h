@@ -68,7 +68,8 @@ int mmf_plan_set_workspace(mmf_plan *plan, void *ws_dev, size_t bytes, void *cud
 
 /* Advance A by nsteps RK4IP steps of size h, Eq. (6a)-(6f), in place.
  *   A_dev  device, [2M][N] complex128 (layout above), 16-byte aligned.  nsteps >= 0 (0 is a no-op).
- * Calling with n1 then n2 steps equals one call with n1+n2 steps. */
+ * Calling with n1 then n2 steps equals one call with n1+n2 steps.  On MMF_ECUDA (a launch failed mid-sequence) the
+ * contents of A_dev and of the workspace are unspecified: the caller must restore the field before retrying. */
 int mmf_propagate(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
 
 /* A link of nspans fibre spans (section 6: "After each span, the fiber losses are compensated by a
@@ -160,8 +161,9 @@ int mmf_debug_freq_index(mmf_plan *plan, long long *idx_host);
 long long mmf_plan_launch_count(const mmf_plan *plan);
 
 /* Per-kernel timing for bench.py's roofline.  mmf_plan_set_timing(plan, 1) makes every later launch of
- * this plan be bracketed by a pair of CUDA events on the launching stream (and drops earlier records); (plan, 0)
- * switches it off.  mmf_plan_get_timing SYNCHRONISES on the recorded events of kernel class `kclass`
+ * this plan be bracketed by a pair of CUDA events on the launching stream (and drops earlier records; at most 65536
+ * launches are recorded, later ones run unrecorded); (plan, 0) switches it off.  While it is on, small problems run
+ * launch by launch instead of from their captured graphs, and without programmatic dependent launch.  mmf_plan_get_timing SYNCHRONISES on the recorded events of kernel class `kclass`
  * (0 <= kclass < mmf_kernel_class_count()) and returns their summed device time [ms], their number, and the
  * ALGORITHMIC bytes of one such launch, averaged over the recorded ones (full-field reads + writes; tables excluded). */
 int mmf_plan_set_timing(mmf_plan *plan, int enable);

@@ -165,13 +165,14 @@ const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", 
                                         "k_shard_apply"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
+constexpr size_t kMaxTimedLaunches = 1 << 16;
 struct LaunchTimer {
   mmf_plan* p;
   cudaStream_t st;
   cudaEvent_t stop = nullptr;
   // nfields = full-field copies the launch reads plus writes (its algorithmic traffic in units of F)
   LaunchTimer(mmf_plan* p_, int kclass, double nfields, cudaStream_t st_) : p(p_), st(st_) {
-    if (!p->timing) return;
+    if (!p->timing || p->ev_class.size() >= kMaxTimedLaunches) return;   // bounded: later launches go unrecorded
     cudaEvent_t a = nullptr;
     if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&stop) != cudaSuccess) { stop = nullptr; return; }
     p->ev.push_back(a);
