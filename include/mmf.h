@@ -68,7 +68,9 @@ int mmf_plan_set_workspace(mmf_plan *plan, void *ws_dev, size_t bytes, void *cud
 
 /* Advance A by nsteps RK4IP steps of size h, Eq. (6a)-(6f), in place.
  *   A_dev  device, [2M][N] complex128 (layout above), 16-byte aligned.  nsteps >= 0 (0 is a no-op).
- * Calling with n1 then n2 steps equals one call with n1+n2 steps.  On MMF_ECUDA (a launch failed mid-sequence) the
+ * Calling with n1 then n2 steps equals one call with n1+n2 steps.  For N = 4096 and M <= 4 the whole call is one
+ * kernel (a thread-block cluster with the field in distributed shared memory; MMF_SMALL_CLUSTER=0 in the environment
+ * selects the kernel-per-stage plan instead).  On MMF_ECUDA (a launch failed mid-sequence) the
  * contents of A_dev and of the workspace are unspecified: the caller must restore the field before retrying. */
 int mmf_propagate(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
 

@@ -14,6 +14,7 @@
 #include "nl_simt.cuh"
 #include "nl_general.cuh"
 #include "nl_shard.cuh"
+#include "small_cluster.cuh"
 
 using namespace mmf;
 
@@ -140,6 +141,7 @@ struct mmf_plan {
   std::vector<OccEntry> occ_cache;
   bool dry_run = false;              // launch helpers prepare (attributes, maps) but do not launch
   bool pdl = true;                   // launch with programmatic stream serialization (async_copy.cuh); MMF_PDL=0 disables
+  int small_cluster = -1;            // whole-propagation cluster kernel (small_cluster.cuh): -1 untested, 0 no, 1 yes
   cudaStream_t cap_stream = nullptr; // capture stream of the step-body graphs
   struct GraphEntry { const void* X; const void* Y; int reps; long long nlaunch; cudaGraphExec_t exec; };
   std::vector<GraphEntry> graphs;
@@ -156,13 +158,13 @@ namespace {
 // ---- kernel classes (for mmf_plan_get_timing) ----------------------------------------------------------------------
 enum { KC_COLS_FWD = 0, KC_ROWS, KC_COLS_INV, KC_NL_PLAIN, KC_NL_STAGE2, KC_NL_STAGE3, KC_NL_FINAL, KC_NL_FINAL_NEXT,
        KC_NLM_PLAIN, KC_NLM_S23, KC_NLM_FINAL, KC_NLM_FINAL_NEXT, KC_NLM_RK4, KC_NLM_ENTER, KC_NLM_EXIT, KC_NLM_AGR_S0,
-       KC_NLM_AGR_IT1, KC_NLM_AGR_ITJ, KC_PERM, KC_NLG_PLAIN, KC_NLG_STAGE2, KC_NLG_STAGE3, KC_NLG_FINAL, KC_SHARD_POW, KC_SHARD_APPLY, KC_COUNT };
+       KC_NLM_AGR_IT1, KC_NLM_AGR_ITJ, KC_PERM, KC_NLG_PLAIN, KC_NLG_STAGE2, KC_NLG_STAGE3, KC_NLG_FINAL, KC_SHARD_POW, KC_SHARD_APPLY, KC_SMALL, KC_COUNT };
 const char* const kc_names[KC_COUNT] = {"k_cols<fwd>", "k_rows", "k_cols<inv>", "k_nl<plain>", "k_nl<stage2>",
                                         "k_nl<stage3>", "k_nl<final>", "k_nl<final_next>", "k_nlm<plain>",
                                         "k_nlm<s23>", "k_nlm<final>", "k_nlm<final_next>", "k_nlm<rk4>", "k_nlm<enter>",
                                         "k_nlm<exit>", "k_nlm<agr_s0>", "k_nlm<agr_it1>", "k_nlm<agr_itj>", "k_perm",
                                         "k_nlg<plain>", "k_nlg<stage2>", "k_nlg<stage3>", "k_nlg<final>", "k_shard_pow",
-                                        "k_shard_apply"};
+                                        "k_shard_apply", "k_small"};
 
 // event bracket around one launch when timing is on (events go on the launching stream)
 constexpr size_t kMaxTimedLaunches = 1 << 16;
@@ -626,6 +628,74 @@ int launch_nlg(mmf_plan* p, const cpx* F0, const cpx* F1, const cpx* Hin, cpx* H
   return MMF_OK;
 }
 
+// The whole propagation in one cluster kernel (small_cluster.cuh): N = 4096, M <= MMF_SMALL_MAXM, Manakov kappa.
+typedef void (*SmallKernel)(SmallParams);
+SmallKernel small_kernel(int M) {
+  switch (M) {
+    case 1: return k_small<1>;
+    case 2: return k_small<2>;
+    case 3: return k_small<3>;
+    case 4: return k_small<4>;
+    default: return nullptr;
+  }
+}
+bool small_cluster_usable(mmf_plan* p) {
+  if (p->small_cluster >= 0) return p->small_cluster == 1;
+  p->small_cluster = 0;
+  const char* e = getenv("MMF_SMALL_CLUSTER");
+  if (e && e[0] == '0') return false;
+  if (p->logn != MMF_SMALL_LOGN || p->M > MMF_SMALL_MAXM || p->general || p->M_total > 0) return false;
+  const int T = 4 * p->M;
+  SmallKernel k_small = small_kernel(p->M);
+  if (cudaFuncSetAttribute(k_small, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem_bytes()) != cudaSuccess ||
+      (T > 8 && cudaFuncSetAttribute(k_small, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
+    cudaGetLastError();
+    return false;
+  }
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(T, 1, 1);
+  cfg.blockDim = dim3(MMF_SMALL_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = small_smem_bytes();
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = T; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int nclusters = 0;
+  if (cudaOccupancyMaxActiveClusters(&nclusters, k_small, &cfg) != cudaSuccess || nclusters < 1) {
+    cudaGetLastError();
+    return false;
+  }
+  p->small_cluster = 1;
+  return true;
+}
+
+int launch_small(mmf_plan* p, cpx* A, int nsteps, int span, double gain, cudaStream_t st) {
+  SmallParams q;
+  q.A = A; q.E = p->E; q.twtab = p->d_tw2; q.kappa = p->d_kappa;
+  q.hg = p->h * p->gamma; q.gain = gain;
+  q.M = p->M; q.nsteps = nsteps; q.span = span;
+  const int T = 4 * p->M;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(T, 1, 1);
+  cfg.blockDim = dim3(MMF_SMALL_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = small_smem_bytes();
+  cfg.stream = st;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = T; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = (p->pdl && !p->timing) ? 2 : 1;
+  LaunchTimer lt(p, KC_SMALL, 2, st);
+  CU(cudaLaunchKernelEx(&cfg, small_kernel(p->M), q));
+  p->launches++;
+  return MMF_OK;
+}
+
 bool finite_all(const double* v, size_t n) {
   for (size_t i = 0; i < n; ++i)
     if (!std::isfinite(v[i])) return false;
@@ -968,6 +1038,7 @@ static int propagate_impl(mmf_plan* p, void* A_dev, int nsteps, int span, double
     // two full-field buffers X, Y.  N <= 4096: the caller's buffer and the workspace's.  N > 4096: both in the
     // workspace, in blocked order; the first and the last nonlinear kernel read / write the caller's buffer in its
     // natural order, so the layout conversions cost no pass of their own.
+    if (!tiled && small_cluster_usable(p)) return launch_small(p, A, nsteps, span, gain, st);   // one kernel for the call
     cpx *X = tiled ? p->Y : A, *Y = tiled ? p->Z : p->Y;
     // per step: D(X,Y); S23 in place; D(X,Y); FINAL(+NEXT)
     if (tiled) rc = launch_nlm<NLM_ENTER>(p, A, X, st, Y);               // X <- A, Y <- h N(A) A   (6b bracket)

@@ -319,3 +319,47 @@ def test_propagate_host_batch(mmf, torch, orc):
         want = orc.rk4ip(A * s, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, 4)
         assert workloads.rel_l2_per_field(H.numpy(), want).max() <= TOL_FIELD
     pl.propagate_host_batch(hosts[:1], d0, None, 0)                       # one field, zero steps: a round trip
+
+
+# ------------------------------------------------------------------------------- whole-propagation cluster kernel
+@pytest.mark.parametrize("M,steps", [(1, 6), (2, 9), (3, 5), (4, 4)])
+def test_small_cluster_kernel_matches_oracle_and_the_launch_by_launch_plan(mmf, torch, orc, monkeypatch, M, steps):
+    """N = 4096, M <= 4: mmf_propagate runs as ONE cluster kernel (small_cluster.cuh: the field in distributed shared
+    memory, D and N alternating with cluster barriers).  Against the oracle, and against the kernel-per-stage plan
+    (MMF_SMALL_CLUSTER=0), which must give the same field to rounding."""
+    p = workloads.problem(0, M=M, N=1 << 12, steps=steps)
+    A = p.field() * 20.0
+    want = orc.rk4ip(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, steps)
+    assert workloads.rel_l2_per_field(orc.rk4ip(A, p.dt, p.h, p.alpha, p.beta, 0.0, p.kappa, steps), want).min() > 1e-4
+    got = {}
+    for mode in ("1", "0"):
+        monkeypatch.setenv("MMF_SMALL_CLUSTER", mode)
+        pl = plan_for(mmf, p)
+        X = to_dev(torch, A)
+        n0 = pl.launch_count()
+        pl.propagate(X, steps)
+        torch.cuda.synchronize()
+        got[mode] = (X.cpu().numpy(), pl.launch_count() - n0)
+        pl.destroy()
+    assert got["1"][1] == 1 and got["0"][1] > 1                 # one launch for the whole call
+    for mode in ("1", "0"):
+        assert workloads.rel_l2_per_field(got[mode][0], want).max() <= 1e-10
+    assert workloads.rel_l2_per_field(got["1"][0], got["0"][0]).max() <= 1e-13
+
+
+def test_small_cluster_kernel_spans_and_composition(mmf, torch, orc):
+    p = workloads.problem(0, M=2, N=1 << 12, steps=6)
+    A = p.field() * 20.0
+    g = float(np.exp(p.alpha * p.h * 3 / 2))
+    pl = plan_for(mmf, p)
+    X = to_dev(torch, A)
+    pl.propagate_spans(X, 2, 3, g)
+    torch.cuda.synchronize()
+    want = orc.rk4ip_spans(A, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa, 2, 3, g)
+    assert workloads.rel_l2_per_field(X.cpu().numpy(), want).max() <= 1e-10
+    X1, X2 = to_dev(torch, A), to_dev(torch, A)
+    pl.propagate(X1, 6)
+    pl.propagate(X2, 2)
+    pl.propagate(X2, 4)
+    torch.cuda.synchronize()
+    assert torch.equal(X1, X2)                                   # n1 + n2 steps == n1 then n2, bit for bit
