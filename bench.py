@@ -356,8 +356,9 @@ def run_mmf(args):
     if world > 1 and shard is None:                  # replicas: a launch-power sweep, one power per rank
         X *= replicas.amplitude_scale(rank, world)
         H.copy_(X)
-    plan = shard.plan if shard is not None else binding.Plan(
-        p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, p.kappa_general() if general else p.kappa, device=dev, general=general)
+    kappa = p.kappa_general() if general else p.kappa_grouped()[0] if args.kappa == "grouped" else p.kappa
+    plan = shard.plan if shard is not None else binding.Plan(p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, kappa, device=dev,
+                                                              general=general)
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -551,7 +552,8 @@ def run_mmf(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if shard is not None else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_string(p) + (" [general 2M x 2M kappa]" if general else ""),
+            "config": {"workload": workload_string(p) + (" [general 2M x 2M kappa]" if general else "") + (
+                           " [mode-group kappa: %d distinct rows]" % plan.groups() if args.kappa == "grouped" else ""),
                        "method": args.method, "kappa": args.kappa, "l2": "field copy %.1f GiB >> 126 MB L2 (no flush needed)"
                        % (F / 2 ** 30) if F > 4 * 126e6 else "working set near/below L2 size: L2-resident",
                        "parallelism": ("row shards x%d (PAPER.md:99-168: whole rows per rank, all-gather of the mode powers 4x per "
@@ -585,7 +587,7 @@ def main():
                     help="rk4ip (Eq. 6, the headline path), ssfm (SSFM-RK4) or agrawal (SSFM-Agrawal): the symmetric "
                          "split step of Eq. 4 with a Runge-Kutta resp. an iterative nonlinear part")
     ap.add_argument("--niter", type=int, default=2, help="iterations per step of --method agrawal")
-    ap.add_argument("--kappa", default="manakov", choices=["manakov", "general"],
+    ap.add_argument("--kappa", default="manakov", choices=["manakov", "general", "grouped"],
                     help="manakov: kappa [M][M] of Eq. 1 (the headline path); general: the paper's [2M][2M] per-polarisation "
                          "matrix (PAPER.md:176; rk4ip only)")
     ap.add_argument("--shard", action="store_true",

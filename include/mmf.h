@@ -162,6 +162,14 @@ int mmf_debug_freq_index(mmf_plan *plan, long long *idx_host);
 /* Number of kernel launches this plan has enqueued since creation (bench.py's gpu_launches). */
 long long mmf_plan_launch_count(const mmf_plan *plan);
 
+/* Mode groups (section 6: "The modes form strongly coupled groups of modes ... This is taken into account
+ * by choosing the appropriate nonlinear coupling coefficients kappa"; Table 2: 15 groups for 120 modes).  When the
+ * kappa given to mmf_plan_create has only G distinct rows (exact equality; every mode of a group couples to the others
+ * alike), G <= 32 and 2 G <= M, the contraction runs on the G distinct rows and every mode picks its group's result:
+ * G M instead of M M products per time sample, the same values bit for bit.  Returns G, or 0 when the plan contracts
+ * the dense matrix (also with MMF_GROUPED=0 in the environment at plan creation). */
+int mmf_plan_groups(const mmf_plan *plan);
+
 /* Per-kernel timing for bench.py's roofline.  mmf_plan_set_timing(plan, 1) makes every later launch of
  * this plan be bracketed by a pair of CUDA events on the launching stream (and drops earlier records; at most 65536
  * launches are recorded, later ones run unrecorded); (plan, 0) switches it off.  While it is on, small problems run

@@ -18,7 +18,7 @@ SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_create_shard"
            "mmf_shard_apply", "mmf_shard_linear", "mmf_shard_end", "mmf_plan_workspace_bytes", "mmf_plan_set_workspace", "mmf_propagate", "mmf_propagate_ssfm",
            "mmf_propagate_ssfm_agrawal", "mmf_propagate_spans",
            "mmf_propagate_host", "mmf_propagate_host_batch", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
-           "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_set_timing", "mmf_kernel_class_count",
+           "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_groups", "mmf_plan_set_timing", "mmf_kernel_class_count",
            "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version",
            "mmf_probe_fp64", "mmf_probe_tma_copy", "mmf_probe_onchip"]
 
@@ -80,6 +80,8 @@ def lib():
     L.mmf_debug_forward.restype = i
     L.mmf_debug_freq_index.argtypes = [vp, ctypes.POINTER(ll)]
     L.mmf_debug_freq_index.restype = i
+    L.mmf_plan_groups.argtypes = [vp]
+    L.mmf_plan_groups.restype = i
     L.mmf_plan_launch_count.argtypes = [vp]
     L.mmf_plan_launch_count.restype = ll
     L.mmf_plan_set_timing.argtypes = [vp, i]
@@ -248,6 +250,10 @@ class Plan:
         _check(lib().mmf_debug_freq_index(self._h, idx.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong))),
                "mmf_debug_freq_index")
         return idx
+
+    def groups(self):
+        """Number of distinct kappa rows the grouped contraction runs on (0: dense)."""
+        return int(lib().mmf_plan_groups(self._h))
 
     def launch_count(self):
         return int(lib().mmf_plan_launch_count(self._h))

@@ -142,6 +142,10 @@ struct mmf_plan {
   bool dry_run = false;              // launch helpers prepare (attributes, maps) but do not launch
   bool pdl = true;                   // launch with programmatic stream serialization (async_copy.cuh); MMF_PDL=0 disables
   int small_cluster = -1;            // whole-propagation cluster kernel (small_cluster.cuh): -1 untested, 0 no, 1 yes
+  // mode groups (nl_tma.cuh GROUPED): kappa has only G distinct rows; 0 = dense contraction
+  int G = 0;
+  double* d_kappa_g = nullptr;       // [G][M]
+  int* d_group_of = nullptr;         // [M]
   cudaStream_t cap_stream = nullptr; // capture stream of the step-body graphs
   struct GraphEntry { const void* X; const void* Y; int reps; long long nlaunch; cudaGraphExec_t exec; };
   std::vector<GraphEntry> graphs;
@@ -539,10 +543,12 @@ int table_tile_map_build(const mmf_plan* p, const void* base, CUtensorMap* map) 
 // caller's field; AGR_*: A = X, B = Y, C = the real table T; other modes: A = X, B = Y (C unused).
 template <int NK, int MODE>
 int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st, double gain) {
-  auto kern = k_nlt<NK, MODE>;
+  auto kern = p->G > 0 ? k_nlt<NK, MODE, 1> : k_nlt<NK, MODE, 0>;
   constexpr int NARR = nlm_narr<MODE>();
   NltParams q;
-  q.kappa = p->d_kappa;
+  q.kappa = p->G > 0 ? p->d_kappa_g : p->d_kappa;
+  q.group_of = p->d_group_of;
+  q.G = p->G;
   q.hg = p->h * p->gamma;
   q.gain = gain;
   q.M = p->M;
@@ -709,6 +715,8 @@ void free_tables(mmf_plan* p) {
   if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
   p->cap_stream = nullptr;
   cudaFree(p->d_kappa);
+  cudaFree(p->d_kappa_g);
+  cudaFree(p->d_group_of);
   cudaFree(p->d_tw1);
   cudaFree(p->d_tw2);
   cudaFree(p->d_ipt);
@@ -845,6 +853,35 @@ static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, doubl
     if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MMF_ENOMEM : cuda_fail(e); break; }
     e = cudaMemcpy(p->d_kappa, kappa, sizeof(double) * KD * KC, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+    if (p->nlm_nk > 0) {
+      // mode groups: if kappa has few DISTINCT rows (exact equality), the contraction runs on those (nl_tma.cuh GROUPED)
+      const char* eg = getenv("MMF_GROUPED");
+      std::vector<int> group_of(M), rep;
+      for (int a = 0; a < M; ++a) {
+        int gfound = -1;
+        for (size_t gi = 0; gi < rep.size() && gfound < 0; ++gi)
+          if (memcmp(kappa + (size_t)a * M, kappa + (size_t)rep[gi] * M, sizeof(double) * M) == 0) gfound = (int)gi;
+        if (gfound < 0) {
+          gfound = (int)rep.size();
+          rep.push_back(a);
+        }
+        group_of[a] = gfound;
+      }
+      const int G = (int)rep.size();
+      if (!(eg && eg[0] == '0') && G <= MMF_NLM_MAXG && 2 * G <= M) {
+        std::vector<double> kg((size_t)G * M);
+        for (int gi = 0; gi < G; ++gi) memcpy(kg.data() + (size_t)gi * M, kappa + (size_t)rep[gi] * M, sizeof(double) * M);
+        e = cudaMalloc((void**)&p->d_kappa_g, sizeof(double) * kg.size());
+        if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MMF_ENOMEM : cuda_fail(e); break; }
+        e = cudaMemcpy(p->d_kappa_g, kg.data(), sizeof(double) * kg.size(), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+        e = cudaMalloc((void**)&p->d_group_of, sizeof(int) * M);
+        if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MMF_ENOMEM : cuda_fail(e); break; }
+        e = cudaMemcpy(p->d_group_of, group_of.data(), sizeof(int) * M, cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+        p->G = G;
+      }
+    }
     if ((rc = upload_stage_tables(&p->d_tw2, p->logn2)) != MMF_OK) break;
     if (p->logn1 > 0) {
       if ((rc = upload_stage_tables(&p->d_tw1, p->logn1)) != MMF_OK) break;
@@ -1339,6 +1376,8 @@ int mmf_debug_freq_index(mmf_plan* p, long long* idx_host) {
 }
 
 long long mmf_plan_launch_count(const mmf_plan* p) { return p ? p->launches : 0; }
+
+int mmf_plan_groups(const mmf_plan* p) { return p ? p->G : 0; }
 
 int mmf_plan_set_timing(mmf_plan* p, int enable) {
   if (!p) return MMF_EINVAL;

@@ -51,7 +51,9 @@ enum { NLM_PLAIN = 0, NLM_S23 = 1, NLM_FINAL = 2, NLM_FINAL_NEXT = 3, NLM_RK4 = 
 #define MMF_NLM_SLOTS 3       // ring depth
 
 struct NltParams {
-  const double* __restrict__ kappa;  // [M][M] row-major
+  const double* __restrict__ kappa;  // [M][M] row-major; GROUPED kernels: the G distinct rows, [G][M]
+  const int* __restrict__ group_of;  // GROUPED kernels: [M], which distinct row mode a has
+  int G;                             // GROUPED kernels: number of distinct rows; the first ceil(G / 8) warps contract
   double hg;
   double gain;       // FINAL / FINAL_NEXT / EXIT: amplitude factor of a lumped amplifier applied to the new field (1 = none)
   int M;
@@ -80,8 +82,10 @@ __host__ __device__ inline size_t nlt_table_bytes(int M) { return ((size_t)M * M
 __host__ __device__ inline size_t nlt_slot_bytes(int M, int narr, bool table) {
   return (size_t)narr * 2 * M * MMF_NLM_T * sizeof(cpx) + (table ? nlt_table_bytes(M) : 0);
 }
+#define MMF_NLM_MAXG 32   // distinct kappa rows the grouped contraction handles (four warps of eight rows)
 __host__ __device__ inline size_t nlt_smem_bytes(int M, int nk, int narr, bool table) {
-  return MMF_NLM_SLOTS * nlt_slot_bytes(M, narr, table) + (size_t)2 * (4 * nk) * MMF_NLM_PSTRIDE * sizeof(double) + 128;
+  return MMF_NLM_SLOTS * nlt_slot_bytes(M, narr, table) + (size_t)2 * (4 * nk) * MMF_NLM_PSTRIDE * sizeof(double) +
+         (size_t)MMF_NLM_MAXG * MMF_NLM_PSTRIDE * sizeof(double) + 128;
 }
 
 // S = kappa_slab * P  for this warp's 8 rows and the tile's 8 samples (four independent accumulator chains)
@@ -100,12 +104,17 @@ __device__ __forceinline__ double power2(cpx a, cpx b) { return (a.x * a.x + a.y
 __device__ __forceinline__ cpx times_ig(cpx u, double g) { return make_double2(-g * u.y, g * u.x); }  // (i g) u
 __device__ __forceinline__ cpx axpy(double s, cpx a, cpx b) { return make_double2(fma(s, a.x, b.x), fma(s, a.y, b.y)); }
 
+// GROUPED (mode groups, section 6: "The modes form strongly coupled groups of modes ... taken into account by
+// choosing the appropriate nonlinear coupling coefficients kappa"): when kappa has only G << M DISTINCT
+// rows (every mode of a group couples to the others alike), S has only G distinct rows too.  The first ceil(G / 8) warps
+// contract the G distinct rows with P (the same DMMA chains, G M instead of M M products per sample), park the result
+// in shared memory, and after one more barrier every lane picks the row of its mode's group.
 // NK = ceil(M / 4) k-steps of the contraction (compile-time: the kappa fragments are a register array).
 // mapA / mapB: 2-D tensor maps (inner = 2N doubles, outer = 2M rows, box = 16 doubles x 2M rows) of
 //   PLAIN: U / OUT;  other modes: X / Y.  mapC: ENTER / EXIT the caller's field; AGR_*: the table T (inner = N doubles,
 //   outer = M rows, box = 8 doubles x M rows).
 // block = 32 (NW + 1) threads; grid = persistent; dynamic smem = nlt_smem_bytes(M, NK, narr).
-template <int NK, int MODE>
+template <int NK, int MODE, int GROUPED = 0>
 __global__ void __launch_bounds__(512, 1)
 k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
       const __grid_constant__ CUtensorMap mapC, NltParams p) {
@@ -120,7 +129,8 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
   const size_t slot_bytes = tab_off + (TABLE ? nlt_table_bytes(M) : 0);
   double* Pb0 = reinterpret_cast<double*>(smem_raw + MMF_NLM_SLOTS * slot_bytes);
   double* Pb1 = Pb0 + 4 * NK * MMF_NLM_PSTRIDE;
-  uint64_t* full = reinterpret_cast<uint64_t*>(Pb1 + 4 * NK * MMF_NLM_PSTRIDE);
+  double* Sg = Pb1 + 4 * NK * MMF_NLM_PSTRIDE;   // GROUPED: S of the distinct rows, [MMF_NLM_MAXG][PSTRIDE]
+  uint64_t* full = reinterpret_cast<uint64_t*>(Sg + MMF_NLM_MAXG * MMF_NLM_PSTRIDE);
   uint64_t* done = full + MMF_NLM_SLOTS;
 
   if (threadIdx.x == 0) {
@@ -207,11 +217,30 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
 
   // this warp's slab of kappa as A fragments: kf[ks] = kappa[a][4 ks + q]
   double kf[NK];
+  const int krow = GROUPED ? warp * 8 + g : a;   // GROUPED: row of the distinct-row matrix this lane's fragments hold
+  const bool kvalid = GROUPED ? krow < p.G : valid;
 #pragma unroll
   for (int ks = 0; ks < NK; ++ks) {
     const int b = 4 * ks + q;
-    kf[ks] = (valid && b < M) ? p.kappa[(long long)a * M + b] : 0.0;
+    kf[ks] = (kvalid && b < M) ? p.kappa[(long long)krow * M + b] : 0.0;
   }
+  const int grp = (GROUPED && valid) ? p.group_of[a] : 0;
+  // S = kappa P for this lane's mode and samples 2q, 2q + 1 (after the barrier that published P)
+  auto contract = [&](const double* Pbuf, double& s0, double& s1) {
+    if constexpr (GROUPED) {
+      if (warp * 8 < p.G) {   // warp-uniform
+        double t0, t1;
+        nlm_contract<NK>(kf, Pbuf, g, q, t0, t1);
+        if (kvalid) *reinterpret_cast<double2*>(Sg + krow * MMF_NLM_PSTRIDE + 2 * q) = make_double2(t0, t1);
+      }
+      group_barrier(1, gthreads);
+      const double2 sv = *reinterpret_cast<const double2*>(Sg + grp * MMF_NLM_PSTRIDE + 2 * q);
+      s0 = sv.x;
+      s1 = sv.y;
+    } else {
+      nlm_contract<NK>(kf, Pbuf, g, q, s0, s1);
+    }
+  };
   const double third = 1.0 / 3.0, sixth = 1.0 / 6.0;
   const int e0 = (2 * a) * MMF_NLM_T + 2 * q;  // this lane's elements: rows 2a (x), 2a+1 (y), samples 2q, 2q+1
 
@@ -261,7 +290,7 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
               make_double2(power2(u[0][0], u[1][0]), power2(u[0][1], u[1][1]));
         group_barrier(1, gthreads);
         double sr[2];
-        nlm_contract<NK>(kf, Pr, g, q, sr[0], sr[1]);
+        contract(Pr, sr[0], sr[1]);
 #pragma unroll
         for (int pol = 0; pol < 2; ++pol)
 #pragma unroll
@@ -290,7 +319,7 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
           make_double2(power2(u[0][0], u[1][0]), power2(u[0][1], u[1][1]));
     group_barrier(1, gthreads);
     double s[2];
-    nlm_contract<NK>(kf, P1, g, q, s[0], s[1]);
+    contract(P1, s[0], s[1]);
     const double g1[2] = {p.hg * s[0], p.hg * s[1]};
 
     if constexpr (MODE == NLM_AGR_S0 || MODE == NLM_AGR_ITJ) {
@@ -347,7 +376,7 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
             make_double2(power2(v[0][0], v[1][0]), power2(v[0][1], v[1][1]));
       group_barrier(1, gthreads);
       double s2[2];
-      nlm_contract<NK>(kf, Pb1, g, q, s2[0], s2[1]);
+      contract(Pb1, s2[0], s2[1]);
       const double g2[2] = {p.hg * s2[0], p.hg * s2[1]};
       if (valid) {
 #pragma unroll

@@ -69,6 +69,23 @@ class Problem:
         k2 = np.kron(self.kappa, pol)
         return np.ascontiguousarray(k2 * rng.uniform(0.9, 1.1, size=k2.shape))
 
+    def kappa_grouped(self, seed=0):
+        """A mode-group kappa (Table 2: the modes form strongly coupled groups; a graded-index fibre's
+        group g holds g spatial modes, 1 + 2 + ... + 15 = 120): kappa_ab = K[g(a)][g(b)] with K symmetric, unit diagonal
+        and seeded off-diagonals from the config's range — every mode of a group has the same row.
+        Returns (kappa [M][M], group_of [M])."""
+        rng = np.random.default_rng([SEED_BASE, self.cfg, 11, int(seed)])
+        group_of, g = [], 0
+        while len(group_of) < self.M:
+            group_of += [g] * (g + 1)
+            g += 1
+        group_of = np.array(group_of[:self.M])
+        G = int(group_of.max()) + 1
+        klo, khi = self._c["kap"]
+        U = np.triu(rng.uniform(klo, khi, size=(G, G)), 1)
+        K = U + U.T + np.eye(G)
+        return np.ascontiguousarray(K[np.ix_(group_of, group_of)]), group_of
+
     # ---- input waveforms -------------------------------------------------------------------------------
     def row(self, r):
         """Input samples of field r = 2a+p (complex128, length N), seeded per row."""

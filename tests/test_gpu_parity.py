@@ -283,9 +283,11 @@ def test_spans_match_oracle(mmf, torch, orc, cfg, M, logn, nspans, k, general):
     assert workloads.rel_l2_per_field(want, nogain).min() > 0.1
 
 
-def test_graph_replay_is_bit_identical_to_direct_launches(mmf, torch):
+def test_graph_replay_is_bit_identical_to_direct_launches(mmf, torch, monkeypatch):
     """small problems replay their step body from a CUDA graph; with per-launch timing on they launch directly:
-    both must give the same bits, for step counts that mix 16-step graphs, 1-step graphs and the direct tail."""
+    both must give the same bits, for step counts that mix 16-step graphs, 1-step graphs and the direct tail.
+    (The kernel-per-stage plan is selected explicitly: at this size mmf_propagate would run as one cluster kernel.)"""
+    monkeypatch.setenv("MMF_SMALL_CLUSTER", "0")
     p = workloads.problem(0, N=1 << 12)
     A = p.field()
     pl = plan_for(mmf, p)
