@@ -543,12 +543,15 @@ int table_tile_map_build(const mmf_plan* p, const void* base, CUtensorMap* map) 
 // caller's field; AGR_*: A = X, B = Y, C = the real table T; other modes: A = X, B = Y (C unused).
 template <int NK, int MODE>
 int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st, double gain) {
-  auto kern = p->G > 0 ? k_nlt<NK, MODE, 1> : k_nlt<NK, MODE, 0>;
   constexpr int NARR = nlm_narr<MODE>();
+  // mode groups: the grouped kernel where its extra S rows still fit beside the ring (they do not for the largest
+  // three-array split-step slots at M = 120 with many groups: those launches contract the dense matrix)
+  const bool grouped = p->G > 0 && nlt_smem_bytes(p->M, NK, NARR, nlm_has_table<MODE>(), p->G) <= 227 * 1024;
+  auto kern = grouped ? k_nlt<NK, MODE, 1> : k_nlt<NK, MODE, 0>;
   NltParams q;
-  q.kappa = p->G > 0 ? p->d_kappa_g : p->d_kappa;
+  q.kappa = grouped ? p->d_kappa_g : p->d_kappa;
   q.group_of = p->d_group_of;
-  q.G = p->G;
+  q.G = grouped ? p->G : 0;
   q.hg = p->h * p->gamma;
   q.gain = gain;
   q.M = p->M;
@@ -563,7 +566,7 @@ int launch_nlm_t(mmf_plan* p, const cpx* A, cpx* B, cpx* C, cudaStream_t st, dou
     if (!C) return MMF_EINVAL;
     if ((rc = table_tile_map(p, C, &mapC)) != MMF_OK) return rc;
   } else if ((rc = field_tile_map(p, C ? C : B, &mapC)) != MMF_OK) return rc;
-  const size_t smem = nlt_smem_bytes(p->M, NK, NARR, nlm_has_table<MODE>());
+  const size_t smem = nlt_smem_bytes(p->M, NK, NARR, nlm_has_table<MODE>(), q.G);
   const int threads = 32 * (q.NW + 1);
   MMF_ENSURE_SMEM(kern, smem);
   int occ = 1;

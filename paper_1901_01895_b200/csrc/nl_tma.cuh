@@ -83,9 +83,11 @@ __host__ __device__ inline size_t nlt_slot_bytes(int M, int narr, bool table) {
   return (size_t)narr * 2 * M * MMF_NLM_T * sizeof(cpx) + (table ? nlt_table_bytes(M) : 0);
 }
 #define MMF_NLM_MAXG 32   // distinct kappa rows the grouped contraction handles (four warps of eight rows)
-__host__ __device__ inline size_t nlt_smem_bytes(int M, int nk, int narr, bool table) {
+// G: distinct rows of the grouped contraction (0: dense kernel, no room for their S)
+__host__ __device__ inline size_t nlt_sg_bytes(int G) { return (size_t)((G + 7) & ~7) * MMF_NLM_PSTRIDE * sizeof(double); }
+__host__ __device__ inline size_t nlt_smem_bytes(int M, int nk, int narr, bool table, int G = 0) {
   return MMF_NLM_SLOTS * nlt_slot_bytes(M, narr, table) + (size_t)2 * (4 * nk) * MMF_NLM_PSTRIDE * sizeof(double) +
-         (size_t)MMF_NLM_MAXG * MMF_NLM_PSTRIDE * sizeof(double) + 128;
+         nlt_sg_bytes(G) + 128;
 }
 
 // S = kappa_slab * P  for this warp's 8 rows and the tile's 8 samples (four independent accumulator chains)
@@ -129,8 +131,8 @@ k_nlt(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensor
   const size_t slot_bytes = tab_off + (TABLE ? nlt_table_bytes(M) : 0);
   double* Pb0 = reinterpret_cast<double*>(smem_raw + MMF_NLM_SLOTS * slot_bytes);
   double* Pb1 = Pb0 + 4 * NK * MMF_NLM_PSTRIDE;
-  double* Sg = Pb1 + 4 * NK * MMF_NLM_PSTRIDE;   // GROUPED: S of the distinct rows, [MMF_NLM_MAXG][PSTRIDE]
-  uint64_t* full = reinterpret_cast<uint64_t*>(Sg + MMF_NLM_MAXG * MMF_NLM_PSTRIDE);
+  double* Sg = Pb1 + 4 * NK * MMF_NLM_PSTRIDE;   // GROUPED: S of the distinct rows, [G rounded up to 8][PSTRIDE]
+  uint64_t* full = reinterpret_cast<uint64_t*>(Sg + (GROUPED ? ((p.G + 7) & ~7) * MMF_NLM_PSTRIDE : 0));
   uint64_t* done = full + MMF_NLM_SLOTS;
 
   if (threadIdx.x == 0) {

@@ -105,3 +105,24 @@ def test_dense_kappa_is_not_grouped(mmf, torch):
     assert _plan(mmf, p, two).groups() == 2
     many = np.arange(144.0).reshape(12, 12); many[1] = many[0]
     assert _plan(mmf, p, many).groups() == 0                          # 11 distinct rows > M / 2: dense
+
+
+def test_many_groups_at_120_modes_all_paths(mmf, torch, orc):
+    """M = 120 with 32 distinct rows: the largest split-step slots leave no room for the grouped kernel's S rows, so
+    those launches contract the dense matrix (mmf_api.cu); every path must still match the oracle."""
+    p = workloads.problem(3, M=120, N=1 << 13, steps=2)
+    rng = np.random.default_rng(5)
+    group_of = np.arange(120) % 32
+    K = rng.uniform(0.01, 0.5, size=(32, 120))
+    kap = K[group_of]
+    A = p.field() * 6.0
+    pl = _plan(mmf, p, kap)
+    assert pl.groups() == 32
+    for name, fn, ref in (("rk4ip", lambda X: pl.propagate(X, 2), lambda: orc.rk4ip(A, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, 2)),
+                          ("ssfm", lambda X: pl.propagate_ssfm(X, 2), lambda: orc.ssfm_rk4(A, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, 2)),
+                          ("agrawal", lambda X: pl.propagate_ssfm_agrawal(X, 2, niter=3),
+                           lambda: orc.ssfm_agrawal(A, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, 2, niter=3))):
+        X = torch.from_numpy(A).cuda()
+        fn(X)
+        torch.cuda.synchronize()
+        assert workloads.rel_l2_per_field(X.cpu().numpy(), ref()).max() <= 1e-10, name
