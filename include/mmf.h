@@ -31,6 +31,7 @@ extern "C" {
 #define MMF_EINVAL -1   /* bad argument (null pointer, size, non-finite parameter, unset/small workspace, alignment) */
 #define MMF_ENOMEM -2   /* host or device allocation failed */
 #define MMF_ECUDA  -3   /* CUDA runtime / launch error */
+#define MMF_ETOOBIG -4  /* mmf_apply_nonlinear_static only: M * N * 8 bytes exceed MMF_STATIC_SCRATCH_BYTES */
 
 typedef struct mmf_plan mmf_plan; /* opaque */
 
@@ -150,6 +151,34 @@ int mmf_shard_end(mmf_plan *plan, void *cuda_stream);
  *                      U and OUT are device [2M][N] complex128 and may alias exactly (OUT == U) or not at all. */
 int mmf_apply_linear(mmf_plan *plan, void *X_dev, void *cuda_stream);
 int mmf_apply_nonlinear(mmf_plan *plan, const void *U_dev, void *OUT_dev, void *cuda_stream);
+
+/* The nonlinear operator for callers that CANNOT ALLOCATE device memory: OUT <- h N(U) U of Eq. (1), as
+ * mmf_apply_nonlinear computes it, but without a plan and without a workspace.
+ *   Who needs it: a host program that took all of HBM for its own pool at start-up (any later cudaMalloc fails there),
+ *   a framework whose caching allocator must see every device byte, and code in a latency-critical loop, where the
+ *   device-wide synchronisation inside cudaMalloc / cudaFree is not acceptable.  mmf_plan_create and a torch-allocated
+ *   workspace are out of reach for all three; this call needs neither, and itself calls no cudaMalloc, cudaFree or
+ *   allocating library routine.
+ *   M >= 1 modes, N >= 1 samples (any N, no transform is involved), h and gamma finite;
+ *   kappa_dev  DEVICE, [M][M] row-major doubles, kappa_dev[a*M + b] = kappa_ab (the caller's memory, not copied);
+ *   U_dev      device, [2M][N] complex128, the layout documented at the top, 16-byte aligned;
+ *   OUT_dev    device, same shape; may be U_dev itself or must not overlap it at all.
+ * It runs the two-kernel form of the paper's Listing 1 (powers to global memory as a real [M][N]
+ * matrix, then contraction and product); the power matrix goes to a file-scope `static __device__` array of
+ * MMF_STATIC_SCRATCH_BYTES (4 MiB), so M * N <= 524 288 (config 0: 8 192, config 1: 393 216 fit; 120 modes up to
+ * N = 4096).  A larger problem returns MMF_ETOOBIG and launches nothing.  Consequences of the static array:
+ *   - each GPU on which the library's code gets loaded gives up those 4 MiB until the process ends;
+ *   - every call on a device uses the same array.  A call writes all the entries it reads, so leftovers of the
+ *     previous call do no harm and nothing needs clearing, but calls that can overlap on the GPU (different streams or
+ *     host threads) race: issue them into one stream or order them with events;
+ *   - the first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *     current) and may trigger the loading of the module.  Make that first call during set-up, before you begin any
+ *     stream capture.  Later calls only enqueue two kernels on `cuda_stream`.
+ * Results agree with mmf_apply_nonlinear to rounding (the sum over b runs in ascending order here, in tensor-core
+ * fragment order there); on integer-valued data both are exact. */
+#define MMF_STATIC_SCRATCH_BYTES (4u << 20)
+int mmf_apply_nonlinear_static(int M, long long N, double h, double gamma, const double *kappa_dev, const void *U_dev,
+                               void *OUT_dev, void *cuda_stream);
 
 /* Debug / test entry points.
  * mmf_debug_forward:  SPEC <- the plain forward transform of every row of X, SPEC[r][k] = sum_n X[r][n] exp(+2 pi i k n/N),

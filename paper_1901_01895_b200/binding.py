@@ -11,7 +11,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmmf_b200.so")
 
-MMF_OK, MMF_EINVAL, MMF_ENOMEM, MMF_ECUDA = 0, -1, -2, -3
+MMF_OK, MMF_EINVAL, MMF_ENOMEM, MMF_ECUDA, MMF_ETOOBIG = 0, -1, -2, -3, -4
+STATIC_SCRATCH_BYTES = 4 << 20   # MMF_STATIC_SCRATCH_BYTES of include/mmf.h
 
 # every symbol include/mmf.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_create_shard", "mmf_shard_begin", "mmf_shard_powers",
@@ -20,7 +21,7 @@ SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_create_shard"
            "mmf_propagate_host", "mmf_propagate_host_batch", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
            "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_groups", "mmf_plan_set_timing", "mmf_kernel_class_count",
            "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version",
-           "mmf_probe_fp64", "mmf_probe_tma_copy", "mmf_probe_onchip"]
+           "mmf_probe_fp64", "mmf_probe_tma_copy", "mmf_probe_onchip", "mmf_apply_nonlinear_static"]
 
 _lib = None
 
@@ -103,6 +104,8 @@ def lib():
     L.mmf_probe_onchip.restype = i
     L.mmf_probe_tma_copy.argtypes = [vp, sz, ull, ull, ull, u, u, i, i, i, i, ll, i, i, i, dp, dp]
     L.mmf_probe_tma_copy.restype = i
+    L.mmf_apply_nonlinear_static.argtypes = [i, ll, d, d, vp, vp, vp, vp]
+    L.mmf_apply_nonlinear_static.restype = i
     L.mmf_version.argtypes = []
     L.mmf_version.restype = ctypes.c_char_p
     _lib = L
@@ -284,6 +287,26 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+
+def apply_nonlinear_static(kappa, U, OUT, h, gamma, stream=None):
+    """mmf_apply_nonlinear_static: OUT <- h N(U) U for callers that may not allocate device memory (no plan, no
+    workspace; the mode powers go through the library's fixed 4 MiB static device array, so M * N <= 524288).
+    kappa: CUDA float64 tensor [M][M]; U, OUT: CUDA complex128 tensors [2M][N] (OUT may be U).  All three are the
+    caller's; this wrapper only passes their addresses and raises MmfError on a non-zero status (MMF_ETOOBIG when the
+    problem exceeds the static array).  The first call on a device does the one-time set-up: see include/mmf.h."""
+    import torch
+    assert kappa.is_cuda and kappa.dtype == torch.float64 and kappa.is_contiguous() and kappa.dim() == 2
+    M = kappa.shape[0]
+    assert kappa.shape[1] == M
+    for T in (U, OUT):
+        assert T.is_cuda and T.dtype == torch.complex128 and T.is_contiguous() and T.shape[0] == 2 * M
+    assert U.shape == OUT.shape
+    _check(lib().mmf_apply_nonlinear_static(int(M), int(U.shape[1]), float(h), float(gamma),
+                                            ctypes.c_void_p(kappa.data_ptr()), ctypes.c_void_p(U.data_ptr()),
+                                            ctypes.c_void_p(OUT.data_ptr()), _stream_ptr(stream)),
+           "mmf_apply_nonlinear_static")
+    return OUT
 
 
 def raw_create(M, N, dt, h, alpha, beta, K, gamma, kappa, general=False):

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmmf_b200.so")
-SOURCES = [os.path.join(CSRC, "mmf_api.cu"), os.path.join(CSRC, "probes.cu")]
+SOURCES = [os.path.join(CSRC, "mmf_api.cu"), os.path.join(CSRC, "probes.cu"), os.path.join(CSRC, "nl_static.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fft_core.cuh", "fft_kernels.cuh", "nl_tma.cuh", "async_copy.cuh", "nl_simt.cuh", "nl_general.cuh", "nl_shard.cuh", "small_cluster.cuh", "tmem_exchange.cuh", "probes.cu")] + [
     os.path.join(os.path.dirname(HERE), "include", "mmf.h")]
 

@@ -773,6 +773,11 @@ int shard_stage(mmf_plan* p, int stage, bool pow, double* P_all, long long t_fir
 bool shard_ready(const mmf_plan* p) { return p && p->M_total > 0 && p->ws && on_plan_device(p); }
 }  // namespace
 
+namespace mmf {
+// For the library's other translation units (nl_static.cu): keep the text of a CUDA error for mmf_status_string.
+int note_cuda_error(cudaError_t e) { return cuda_fail(e); }
+}  // namespace mmf
+
 extern "C" {
 
 const char* mmf_version(void) { return "mmf-b200 0.1"; }
@@ -783,6 +788,7 @@ const char* mmf_status_string(int status) {
     case MMF_EINVAL: return "invalid argument";
     case MMF_ENOMEM: return "out of memory";
     case MMF_ECUDA: return g_cuda_msg;
+    case MMF_ETOOBIG: return "problem too large for the static scratch array (M * N * 8 > MMF_STATIC_SCRATCH_BYTES)";
     default: return "unknown status";
   }
 }

@@ -50,3 +50,21 @@ def test_missing_library_fails_loudly(mmf, monkeypatch):
     monkeypatch.setattr(mmf, "LIB_PATH", "/nonexistent/libmmf_b200.so")
     with pytest.raises(mmf.MmfError):
         mmf.lib()
+
+
+def test_static_entry_point_validates_before_touching_cuda(mmf):
+    """mmf_apply_nonlinear_static (the entry point that allocates nothing): argument and size checks come before any
+    CUDA call, so they can be exercised without a GPU (the pointers are never dereferenced on these paths)."""
+    import ctypes
+    L = mmf.lib()
+    fake = ctypes.c_void_p(4096)
+    assert L.mmf_apply_nonlinear_static(129, 4096, 1.0, 1.0, fake, fake, fake, None) == mmf.MMF_ETOOBIG
+    assert L.mmf_apply_nonlinear_static(1, (1 << 19) + 1, 1.0, 1.0, fake, fake, fake, None) == mmf.MMF_ETOOBIG
+    assert L.mmf_apply_nonlinear_static(1 << 30, 1 << 40, 1.0, 1.0, fake, fake, fake, None) == mmf.MMF_ETOOBIG
+    assert b"MMF_STATIC_SCRATCH_BYTES" in L.mmf_status_string(mmf.MMF_ETOOBIG)
+    assert L.mmf_apply_nonlinear_static(0, 16, 1.0, 1.0, fake, fake, fake, None) == mmf.MMF_EINVAL
+    assert L.mmf_apply_nonlinear_static(2, 16, 1.0, float("inf"), fake, fake, fake, None) == mmf.MMF_EINVAL
+    assert L.mmf_apply_nonlinear_static(2, 16, 1.0, 1.0, fake, ctypes.c_void_p(4104), fake, None) == mmf.MMF_EINVAL
+    assert L.mmf_apply_nonlinear_static(2, 16, 1.0, 1.0, fake, None, fake, None) == mmf.MMF_EINVAL
+    hdr = open(os.path.join(ROOT, "include", "mmf.h")).read()
+    assert int(re.search(r"#define MMF_STATIC_SCRATCH_BYTES \((\d+)u << (\d+)\)", hdr).group(1)) << 20 == mmf.STATIC_SCRATCH_BYTES
