@@ -71,7 +71,8 @@ int mmf_plan_set_workspace(mmf_plan *plan, void *ws_dev, size_t bytes, void *cud
  *   A_dev  device, [2M][N] complex128 (layout above), 16-byte aligned.  nsteps >= 0 (0 is a no-op).
  * Calling with n1 then n2 steps equals one call with n1+n2 steps.  For N = 4096 and M <= 4 the whole call is one
  * kernel (a thread-block cluster with the field in distributed shared memory; MMF_SMALL_CLUSTER=0 in the environment
- * selects the kernel-per-stage plan instead).  On MMF_ECUDA (a launch failed mid-sequence) the
+ * selects the kernel-per-stage plan instead; the two agree to rounding — <= 1e-13 relative L2 per field in the tests —
+ * not bit for bit, because the cluster kernel sums kappa_ab P_b in a per-warp rotated mode order).  On MMF_ECUDA (a launch failed mid-sequence) the
  * contents of A_dev and of the workspace are unspecified: the caller must restore the field before retrying. */
 int mmf_propagate(mmf_plan *plan, void *A_dev, int nsteps, void *cuda_stream);
 
@@ -135,6 +136,9 @@ int mmf_propagate_host_batch(mmf_plan *plan, void *const *A_hosts, int nfields, 
  *   caller's all-gather fills the other rows; apply reads all of them.  Chunks let the gather of one chunk overlap
  *   the kernels of its neighbours.  For N > 4096 the sample index is the library's internal (blocked)
  *   order — the same on every rank, since it depends on N only.  stage: 0..3 as listed.
+ * Size bound, checked by mmf_plan_create_shard (MMF_EINVAL): the apply kernel keeps the rank's kappa rows, a power tile
+ *   and a result tile in one SM's shared memory, 8 (M_total MP + 32 M_total + 32 MP) <= 232 448 bytes with MP = M_local
+ *   rounded up to a multiple of 4 (e.g. M_total = 240: M_local <= 80, three ranks or more; M_total = 120: any split).
  * Shard plans accept only the mmf_shard_* calls, mmf_apply_linear and the timing / debug calls. */
 int mmf_plan_create_shard(mmf_plan **out, int M_local, int M_total, int mode0, long long N, double dt, double h,
                           double alpha, const double *beta, int K, double gamma, const double *kappa_rows);

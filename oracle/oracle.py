@@ -17,7 +17,11 @@ _lib = None
 
 
 def build(force=False):
-    """Compile oracle/rk4ip_oracle.cpp -> oracle/liboracle.so (plain g++, no fast-math)."""
+    """Compile oracle/rk4ip_oracle.cpp -> oracle/liboracle.so (plain g++, no fast-math).
+    MMF_ORACLE_LIB in the environment names a library built otherwise from the same source (tests/test_oracle_sanitized.py
+    runs the pins on an -fsanitize=address,undefined build); it is then loaded as it is."""
+    if os.environ.get("MMF_ORACLE_LIB"):
+        return os.environ["MMF_ORACLE_LIB"]
     if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
         return _LIB
     tmp = _LIB + ".tmp.%d" % os.getpid()

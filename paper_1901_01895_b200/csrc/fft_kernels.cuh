@@ -386,7 +386,6 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
   constexpr uint32_t TMEM_COLS = 4 * WARP_COLS;  // 4 warps share a lane quarter
   uint32_t* tmem_word = reinterpret_cast<uint32_t*>(done + G);
   uint64_t* tabbar = done + G + 1;
-  pdl_launch_dependents();
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
@@ -404,6 +403,10 @@ k_rows(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtenso
     tmem_fence_before_sync();
   }
   __syncthreads();
+  // Dependents are released only now, with the tensor-memory columns in hand: a successor that allocates tensor memory
+  // ahead of its own griddepcontrol.wait could otherwise land on this SM, take the columns first and then wait for a
+  // grid whose CTA here is still blocked in tcgen05.alloc.  A kernel signals once it holds every blocking resource.
+  pdl_launch_dependents();
   pdl_wait();                            // the field buffers (and, after plan set-up, the E table) come from predecessors
   uint32_t taddr = 0;   // this warp's columns: [0, 64) the E values of the item, [64, 128) the exchange buffer (TMX)
   if constexpr (ECACHE || TMX) {

@@ -6,6 +6,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <mutex>
 #include <vector>
 
 #include "../../include/mmf.h"
@@ -136,7 +137,6 @@ struct mmf_plan {
   // body of small problems is replayed from a captured CUDA graph
   struct MapEntry { int kind; const void* base; int aux; CUtensorMap map; };
   std::vector<MapEntry> map_cache;
-  std::vector<const void*> attr_done;
   struct OccEntry { const void* kern; int threads; size_t smem; int occ; };
   std::vector<OccEntry> occ_cache;
   bool dry_run = false;              // launch helpers prepare (attributes, maps) but do not launch
@@ -315,14 +315,32 @@ int field_tile_map(mmf_plan* p, const void* base, CUtensorMap* map, int boxrows 
 }
 int table_tile_map(mmf_plan* p, const void* base, CUtensorMap* map) { return cached_map(p, MAP_TABLE, base, 0, map); }
 
-// cudaFuncAttributeMaxDynamicSharedMemorySize, once per plan and kernel
+// cudaFuncAttributeMaxDynamicSharedMemorySize.  The attribute belongs to the (kernel, device) pair, not to a plan, and
+// several kernels' dynamic shared memory depends on plan values (M, G, the shard sizes), so two live plans can share an
+// instantiation with different needs.  The library therefore keeps, process-wide, the largest value it has set per
+// kernel and device and only ever RAISES it: a launch with a smaller need is covered by the larger opt-in, and no plan
+// can lower the limit under another one.  (A per-plan "done" flag is only a shortcut in front of the shared record.)
+struct SmemAttr {
+  const void* kern;
+  int device;
+  size_t bytes;
+};
+std::mutex g_smem_attr_mutex;
+std::vector<SmemAttr> g_smem_attr;
+
 template <class K>
 int ensure_smem(mmf_plan* p, K kern, size_t smem) {
   const void* key = reinterpret_cast<const void*>(kern);
-  for (const void* k : p->attr_done)
-    if (k == key) return MMF_OK;
+  std::lock_guard<std::mutex> lock(g_smem_attr_mutex);
+  for (SmemAttr& a : g_smem_attr)
+    if (a.kern == key && a.device == p->device) {
+      if (smem <= a.bytes) return MMF_OK;
+      CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      a.bytes = smem;
+      return MMF_OK;
+    }
   CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  p->attr_done.push_back(key);
+  g_smem_attr.push_back({key, p->device, smem});
   return MMF_OK;
 }
 template <class K>
@@ -826,6 +844,9 @@ static int plan_create_impl(mmf_plan** out, int M, long long N, double dt, doubl
   if (general && M > MMF_NLG_MAXM) return MMF_EINVAL;       // the general kernel keeps an M x 2M slab in tensor memory
   if (!finite_all(beta, (size_t)M * K) || !finite_all(kappa, KD * KC)) return MMF_EINVAL;
   if (sizeof(double) * 2 * KC * MMF_NL_T > 227 * 1024) return MMF_EINVAL;  // mode-power tile must fit one SM
+  // a shard plan's apply kernel keeps the rank's kappa rows, a power tile and a result tile in one SM's shared memory:
+  // refuse here, not at the first mmf_shard_apply in the middle of a step (include/mmf.h states the bound)
+  if (shard && shard_apply_smem_bytes(M, M_total) > 227 * 1024) return MMF_EINVAL;
   mmf_plan* p = new (std::nothrow) mmf_plan;
   if (!p) return MMF_ENOMEM;
   p->M = M; p->K = K; p->N = N; p->dt = dt; p->h = h; p->alpha = alpha; p->gamma = gamma;

@@ -69,8 +69,13 @@ __device__ __forceinline__ void st_cluster(uint32_t addr, cpx v) {
 
 enum { SM_PLAIN = 0, SM_S23 = 1, SM_FINAL = 2, SM_FINAL_NEXT = 3 };
 
-// S_a = sum_b kappa_ab P_b for the M <= 4 modes of one sample (b ascending, as the oracle sums)
-// P, S are held in ROTATED positions: position a' is mode (a' + q) mod M (see small_nl_phase).
+// S_a = sum_b kappa_ab P_b for the M <= 4 modes of one sample.
+// P, S are held in ROTATED positions: position a' is mode (a' + q) mod M (see small_nl_phase), and the sum runs over
+// the positions in ascending order, i.e. over the modes in the order q, q + 1, ..., M - 1, 0, ..., q - 1 with q
+// depending on CTA and warp.  That is NOT the oracle's b-ascending order: the result agrees with the oracle and with
+// the kernel-per-stage plan to rounding (a few ulp of S), not bit for bit, and the rounding of a sample depends on the
+// warp that owns it.  (include/mmf.h says so; test_small_cluster_kernel_matches_oracle_and_the_launch_by_launch_plan
+// bounds the difference at 1e-13 relative L2 per field.)
 template <int M>
 __device__ __forceinline__ void small_contract(const double* __restrict__ kap, int q, const double (&P)[M], double (&S)[M]) {
 #pragma unroll
@@ -207,7 +212,6 @@ __global__ void __launch_bounds__(MMF_SMALL_THREADS, 1) k_small(SmallParams p) {
   const int row = (int)c % R;
   const bool is_x = (int)c < R;
 
-  pdl_launch_dependents();
   if (t == 0) {
     mbar_init(tabbar, 1);
     mbar_init_fence();
@@ -222,6 +226,7 @@ __global__ void __launch_bounds__(MMF_SMALL_THREADS, 1) k_small(SmallParams p) {
   if (t < M * M) kap[t] = p.kappa[t];
   __syncthreads();
   tmem_fence_after_sync();
+  pdl_launch_dependents();   // after tcgen05.alloc, never before: see k_rows (a chain of these kernels allocates 256 columns each)
   pdl_wait();
   const uint32_t warp = (uint32_t)t >> 5;
   const uint32_t taddr = *tmem_word + (((warp & 3) * 32) << 16) + (warp >> 2) * 128;

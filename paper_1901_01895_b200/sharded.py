@@ -114,15 +114,17 @@ def propagate(stages, A, nsteps, gather, span=0, gain=1.0):
     if nsteps <= 0:
         return A
     stages.begin(A)
-    evaluate(stages, SH_PLAIN, gather)                 # bracket of (6b): h N(A) A
-    for s in range(nsteps):
-        stages.linear(0)                               # (6a) A_I, (6b) k1
-        evaluate(stages, SH_STAGE2, gather)            # (6c) k2
-        evaluate(stages, SH_STAGE3, gather)            # (6d) k3 and the brackets of (6e), (6f)
-        stages.linear(1)                               # (6e) argument u4, (6f) first term
-        g = gain if (span > 0 and (s + 1) % span == 0) else 1.0
-        evaluate(stages, SH_FINAL, gather, g)          # (6e) + (6f): the new field
-        if s + 1 < nsteps:
-            evaluate(stages, SH_PLAIN, gather)         # the next step's (6b) bracket
-    stages.end()
+    try:
+        evaluate(stages, SH_PLAIN, gather)                 # bracket of (6b): h N(A) A
+        for s in range(nsteps):
+            stages.linear(0)                               # (6a) A_I, (6b) k1
+            evaluate(stages, SH_STAGE2, gather)            # (6c) k2
+            evaluate(stages, SH_STAGE3, gather)            # (6d) k3 and the brackets of (6e), (6f)
+            stages.linear(1)                               # (6e) argument u4, (6f) first term
+            g = gain if (span > 0 and (s + 1) % span == 0) else 1.0
+            evaluate(stages, SH_FINAL, gather, g)          # (6e) + (6f): the new field
+            if s + 1 < nsteps:
+                evaluate(stages, SH_PLAIN, gather)         # the next step's (6b) bracket
+    finally:
+        stages.end()                                   # also after a failed stage: the plan must not keep A attached
     return A

@@ -68,3 +68,20 @@ def test_static_entry_point_validates_before_touching_cuda(mmf):
     assert L.mmf_apply_nonlinear_static(2, 16, 1.0, 1.0, fake, None, fake, None) == mmf.MMF_EINVAL
     hdr = open(os.path.join(ROOT, "include", "mmf.h")).read()
     assert int(re.search(r"#define MMF_STATIC_SCRATCH_BYTES \((\d+)u << (\d+)\)", hdr).group(1)) << 20 == mmf.STATIC_SCRATCH_BYTES
+
+
+def test_shard_plan_that_cannot_run_its_apply_kernel_is_refused_at_creation(mmf):
+    """A shard plan whose kappa rows + tiles exceed one SM's shared memory (include/mmf.h states the bound) must fail in
+    mmf_plan_create_shard, not at the first mmf_shard_apply in the middle of a step."""
+    import ctypes
+    L = mmf.lib()
+    dp = ctypes.POINTER(ctypes.c_double)
+    for M_local, M_total in ((120, 240), (80, 240)):
+        MP = (M_local + 3) & ~3
+        assert 8 * (M_total * MP + 32 * M_total + 32 * MP) > 227 * 1024
+        h = ctypes.c_void_p()
+        beta = np.zeros((M_local, 1))
+        kap = np.ones((M_local, M_total))
+        rc = L.mmf_plan_create_shard(ctypes.byref(h), M_local, M_total, 0, 4096, 1.0, 1.0, 0.0, beta.ctypes.data_as(dp), 1,
+                                     1.0, kap.ctypes.data_as(dp))
+        assert rc == mmf.MMF_EINVAL and not h.value

@@ -36,3 +36,24 @@ def test_reference_arm_times_the_split_step_oracles_too():
     for method in ("ssfm", "agrawal"):
         d = _run("--method", method)
         assert d["config"]["method"] == method and d["value"] > 0
+
+
+def test_gpus_n_starts_n_ranks_by_itself():
+    """`python bench.py --gpus 2` without a torchrun environment must start 2 ranks (one per GPU on the box); here the
+    --dry-run leg (gloo, no CUDA) checks the launcher and the aggregation: n_gpus = 2, units summed, time = max."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "4", "--cfg", "0",
+                          "--dry-run"], capture_output=True, text=True, timeout=300, env=env, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, out.stdout                      # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["dry_run"] and d["n_gpus"] == 2 and d["gpus_requested"] == 2
+    assert d["units"] == 2 * 4 * 4096 * 4                   # 2 ranks x (R = 4 rows x N = 4096) x 4 steps
+    assert abs(d["ms_per_step"] - 110.0) < 1e-9             # the slower rank's (synthetic) time
+    assert abs(d["value"] - d["units"] / 0.44) < 1e-3

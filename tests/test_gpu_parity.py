@@ -365,3 +365,36 @@ def test_small_cluster_kernel_spans_and_composition(mmf, torch, orc):
     pl.propagate(X2, 4)
     torch.cuda.synchronize()
     assert torch.equal(X1, X2)                                   # n1 + n2 steps == n1 then n2, bit for bit
+
+
+# ------------------------------------------------------------------------------------ several live plans at once
+def test_two_live_plans_sharing_a_kernel_instantiation_interleave(mmf, torch, orc):
+    """The opt-in shared-memory limit is a property of (kernel, device), not of a plan.  Two live plans whose launches
+    go through the same kernel instantiation with DIFFERENT dynamic shared-memory sizes (M = 8 and M = 7 share one
+    k_nlt bucket; two general plans with different M share k_nlg; two M > 120 plans share k_nl) must keep working when
+    their calls alternate: the library may only ever raise that limit."""
+    def run(cases, **kw):
+        plans, fields, wants = [], [], []
+        for cfg, M, scale in cases:
+            p = workloads.problem(cfg, M=M, N=1 << 13, steps=2)
+            A = p.field() * scale
+            kap = p.kappa
+            if kw.get("general"):
+                kap = p.kappa_general(M)
+                wants.append(orc.rk4ip_general(A, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, 4))
+            else:
+                wants.append(orc.rk4ip(A, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, 4))
+            plans.append(mmf.Plan(p.M, p.N, p.dt, p.h, p.alpha, p.beta, p.gamma, kap, **kw))
+            fields.append(to_dev(torch, A))
+        for _ in range(2):                      # larger first, then smaller, then larger again ...
+            for pl, X in zip(plans, fields):
+                pl.propagate(X, 2)
+        torch.cuda.synchronize()
+        for X, want in zip(fields, wants):
+            assert np.isfinite(want).all()
+            assert workloads.rel_l2_per_field(X.cpu().numpy(), want).max() <= TOL_FIELD
+        for pl in plans:
+            pl.destroy()
+    run(((1, 8, 10.0), (1, 7, 10.0)))
+    run(((3, 124, 1.0), (3, 122, 1.0)))
+    run(((1, 9, 3.0), (1, 5, 3.0)), general=True)

@@ -137,3 +137,32 @@ def test_single_process_gather_is_a_no_op():
     assert sharded.chunk_ranges(256, 4) == [(0, 64), (64, 64), (128, 64), (192, 64)]
     with pytest.raises(ValueError):
         sharded.chunk_ranges(256, 16)
+
+
+def test_propagate_detaches_the_field_when_a_stage_fails():
+    """sharded.propagate calls stages.end() in a finally block: a stage that raises must not leave A attached."""
+    from paper_1901_01895_b200 import sharded
+
+    class Failing:
+        ranges = [(0, 16)]
+        log = []
+
+        def begin(self, A):
+            self.log.append("begin")
+
+        def powers(self, stage, c=0):
+            self.log.append("powers")
+
+        def apply(self, stage, c=0, gain=1.0):
+            raise RuntimeError("apply failed")
+
+        def linear(self, which):
+            self.log.append("linear")
+
+        def end(self):
+            self.log.append("end")
+
+    st = Failing()
+    with pytest.raises(RuntimeError, match="apply failed"):
+        sharded.propagate(st, None, 2, lambda c: None)
+    assert st.log == ["begin", "powers", "end"]
