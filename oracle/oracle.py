@@ -49,6 +49,11 @@ def lib():
         L.orc_rk4ip_general.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i]
         L.orc_rk4ip_spans.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i, i, d, i]
         L.orc_ssfm_agrawal.argtypes = [dp, i, ll, d, d, d, dp, i, d, dp, i, i, i]
+        u32p = ctypes.POINTER(ctypes.c_uint32)
+        L.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]
+        L.orc_noise_unit.argtypes = [dp, ctypes.c_ulonglong, ctypes.c_uint, ctypes.c_ulonglong, ll]
+        L.orc_add_noise.argtypes = [dp, i, ll, d, d, d, i, ctypes.c_ulonglong, dp]
+        L.orc_philox4x32_10.restype = L.orc_noise_unit.restype = L.orc_add_noise.restype = i
         for f in (L.orc_dft, L.orc_fft, L.orc_omega, L.orc_linear_table, L.orc_apply_D, L.orc_nonlinear,
                   L.orc_rk4ip, L.orc_ssfm_rk4, L.orc_ssfm_agrawal, L.orc_nonlinear_general, L.orc_rk4ip_general, L.orc_rk4ip_spans):
             f.restype = i
@@ -203,3 +208,32 @@ def rk4ip_spans(A, dt, h, alpha, beta, gamma, kappa, nspans, steps_per_span, gai
                                nspans, steps_per_span, gain, nthreads)
     assert rc == 0, "orc_rk4ip_spans rejected its arguments"
     return A
+
+
+def philox4x32_10(ctr, key):
+    """The Philox-4x32-10 block function: 4 counter words, 2 key words -> 4 output words (uint32 arrays)."""
+    c = np.ascontiguousarray(ctr, dtype=np.uint32)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.empty(4, dtype=np.uint32)
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    assert c.size == 4 and k.size == 2
+    assert lib().orc_philox4x32_10(c.ctypes.data_as(u32p), k.ctypes.data_as(u32p), out.ctypes.data_as(u32p)) == 0
+    return out
+
+
+def noise_unit(seed, row, t0, count):
+    """The unit complex normal samples z(row, t0 .. t0 + count - 1) of the noise stream `seed` (E|z|^2 = 1)."""
+    z = np.empty(count, dtype=np.complex128)
+    assert lib().orc_noise_unit(_p(z), int(seed), int(row), int(t0), int(count)) == 0
+    return z
+
+
+def add_noise(A, dt, osnr_db, ref_bw, nch, seed):
+    """Noise loading (reading R18): returns (A + noise, mean power per spatial mode before the noise)."""
+    A = _c128(A).copy()
+    R, N = A.shape
+    M = R // 2
+    P = np.empty(M, dtype=np.float64)
+    rc = lib().orc_add_noise(_p(A), M, N, float(dt), float(osnr_db), float(ref_bw), int(nch), int(seed), _p(P))
+    assert rc == 0, "orc_add_noise rejected its arguments"
+    return A, P

@@ -27,6 +27,14 @@
 // soliton shape, 4th-order convergence against an independent adaptive integrator, integer exactness,
 // composition.  No function here is "parity unpinned".
 //
+// Noise loading (section 6: "White noise is added to the signals before the receiver, setting the optical
+// signal-to-noise ratio (OSNR) to 20 dB"; reading R18 in DESIGN.md): philox4x32_10 (the counter-based generator of
+// Salmon, Moraes, Dror, Shaw, "Parallel random numbers: as easy as 1, 2, 3", SC'11, written from its definition),
+// gaussian_pair (Box-Muller) and add_noise.  Pins (tests/test_oracle_noise_pins.py): the generator's published
+// known-answer vectors bit for bit, uniform-to-unit-interval mapping limits, mean / variance / whiteness / normality of
+// the added field within stated statistical bounds, the realised OSNR of a known-power field, the zero-noise limit,
+// stream independence of the matrix size.
+//
 // Numerical hygiene: twiddles and the dispersion phase are evaluated per index in long double
 // (never by recurrence); no -ffast-math.
 
@@ -332,6 +340,76 @@ void ssfm_agrawal_step(cplx* A, int M, long long N, const cplx* E, double hgamma
   std::memcpy((void*)A, (const void*)Y, sizeof(cplx) * tot);
 }
 
+
+// ------------------------------------------------------------------------------------------------ noise loading
+// Philox-4x32 with 10 rounds (Salmon et al., SC'11, section 3.3 / Table 2): the state is four 32-bit words c0..c3, the
+// key two words k0, k1.  One round: (hi0, lo0) = M0 * c0, (hi1, lo1) = M1 * c2 (32 x 32 -> 64-bit products), then
+//   c0' = hi1 ^ c1 ^ k0,  c1' = lo1,  c2' = hi0 ^ c3 ^ k1,  c3' = lo0;
+// between rounds the key is bumped by the Weyl constants W0 (golden ratio), W1 (sqrt(3) - 1).
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  const uint64_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+  const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    if (round > 0) {
+      k0 += W0;
+      k1 += W1;
+    }
+    const uint64_t p0 = M0 * c0, p1 = M1 * c2;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0, hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    const uint32_t n0 = hi1 ^ c1 ^ k0, n1 = lo1, n2 = hi0 ^ c3 ^ k1, n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Two 32-bit words -> a double in the OPEN interval (0, 1): the top 52 bits k of (hi : lo), u = (k + 1/2) 2^-52.
+// Every value is exactly representable (k + 1/2 has at most 53 significant bits); smallest 2^-53, largest 1 - 2^-53.
+double unit_open(uint32_t hi, uint32_t lo) {
+  const uint64_t k = ((uint64_t)hi << 20) | (uint64_t)(lo >> 12);
+  return ((double)k + 0.5) * 0x1p-52;
+}
+
+// The complex standard normal sample (E|z|^2 = 1, real and imaginary part independent N(0, 1/2)) of row r, sample t
+// under `seed`: counter = (t low word, t high word, r, 0), key = (seed low word, seed high word); Box-Muller on
+// u1 = unit_open(w0, w1), u2 = unit_open(w2, w3):  z = sqrt(-ln u1) (cos 2 pi u2 + i sin 2 pi u2).
+cplx noise_unit_sample(uint64_t seed, uint32_t row, uint64_t t) {
+  const uint32_t ctr[4] = {(uint32_t)t, (uint32_t)(t >> 32), row, 0u};
+  const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  uint32_t w[4];
+  philox4x32_10(ctr, key, w);
+  const double u1 = unit_open(w[0], w[1]), u2 = unit_open(w[2], w[3]);
+  const double rad = std::sqrt(-std::log(u1));
+  const long double ang = 6.283185307179586476925286766559005768L * (long double)u2;
+  return cplx(rad * (double)cosl(ang), rad * (double)sinl(ang));
+}
+
+// PAPER.md:255 with reading R18.  For every spatial mode a:
+//   P_a     = (1/N) sum_t (|A_ax(t)|^2 + |A_ay(t)|^2)          mean signal power of the mode, both polarisations [W]
+//   P_ch    = P_a / nch                                         per wavelength channel (nch channels share the mode)
+//   N0      = P_ch / (2 B_ref OSNR)                             noise power spectral density PER POLARISATION: the OSNR
+//                                                               counts the noise of both polarisations in B_ref
+//   sigma^2 = N0 / dt                                           variance of one complex sample of one polarisation: white
+//                                                               over the whole simulated band 1/dt
+//   A_{a,p}(t) += sigma_a z_{2a+p}(t),  z = noise_unit_sample.
+// power_out[a] = P_a (of the field BEFORE the noise).  OSNR = 10^(osnr_db/10); osnr_db = +inf adds nothing.
+void add_noise(cplx* A, int M, long long N, double dt, double osnr_db, double ref_bw, int nch, uint64_t seed,
+               double* power_out) {
+  const double osnr = std::pow(10.0, osnr_db / 10.0);
+  for (int a = 0; a < M; ++a) {
+    double sum = 0.0;
+    for (int p = 0; p < 2; ++p)
+      for (long long t = 0; t < N; ++t) sum += std::norm(A[(size_t)(2 * a + p) * N + t]);
+    const double P = sum / (double)N;
+    power_out[a] = P;
+    const double sigma = std::sqrt(P / (double)nch / (2.0 * ref_bw * osnr) / dt);
+    if (!(sigma > 0.0)) continue;
+    for (int p = 0; p < 2; ++p)
+      for (long long t = 0; t < N; ++t)
+        A[(size_t)(2 * a + p) * N + t] += sigma * noise_unit_sample(seed, (uint32_t)(2 * a + p), (uint64_t)t);
+  }
+}
+
 }  // namespace
 
 extern "C" {
@@ -462,6 +540,30 @@ int orc_ssfm_agrawal(double* A, int M, long long N, double dt, double h, double 
   for (int s = 0; s < nsteps; ++s)
     ssfm_agrawal_step((cplx*)A, M, N, E.data(), h * gamma, kappa, niter, nthreads, B.data(), Y.data(), S0.data(),
                       S1.data());
+  return 0;
+}
+
+// noise loading: the generator alone (for its known-answer pins) and the whole operation
+int orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
+  if (!ctr || !key || !out) return -1;
+  philox4x32_10(ctr, key, out);
+  return 0;
+}
+
+int orc_noise_unit(double* z, unsigned long long seed, unsigned row, unsigned long long t0, long long count) {
+  if (!z || count < 0) return -1;
+  for (long long i = 0; i < count; ++i) {
+    const cplx v = noise_unit_sample(seed, row, t0 + (uint64_t)i);
+    z[2 * i] = v.real();
+    z[2 * i + 1] = v.imag();
+  }
+  return 0;
+}
+
+int orc_add_noise(double* A, int M, long long N, double dt, double osnr_db, double ref_bw, int nch,
+                  unsigned long long seed, double* power_out) {
+  if (!A || !power_out || M < 1 || N < 1 || !(dt > 0) || !(ref_bw > 0) || nch < 1 || std::isnan(osnr_db)) return -1;
+  add_noise(reinterpret_cast<cplx*>(A), M, N, dt, osnr_db, ref_bw, nch, seed, power_out);
   return 0;
 }
 

@@ -20,7 +20,7 @@ def test_oracle_pins_pass_under_asan_and_ubsan(tmp_path):
                ASAN_OPTIONS="detect_leaks=0:abort_on_error=1", UBSAN_OPTIONS="halt_on_error=1:print_stacktrace=1")
     # the pins of every oracle function; the two long ones (step-size table, 2^22 transform) add nothing for this purpose
     out = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider",
-                          "tests/test_oracle_pins.py", "tests/test_oracle_ssfm_pins.py", "tests/test_oracle_general_pins.py",
+                          "tests/test_oracle_pins.py", "tests/test_oracle_ssfm_pins.py", "tests/test_oracle_general_pins.py", "tests/test_oracle_noise_pins.py",
                           "-k", "not stepsize_table_claim and not full_length"],
                          cwd=ROOT, env=env, capture_output=True, text=True, timeout=900)
     tail = out.stdout[-3000:] + out.stderr[-3000:]
