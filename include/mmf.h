@@ -156,6 +156,27 @@ int mmf_shard_end(mmf_plan *plan, void *cuda_stream);
 int mmf_apply_linear(mmf_plan *plan, void *X_dev, void *cuda_stream);
 int mmf_apply_nonlinear(mmf_plan *plan, const void *U_dev, void *OUT_dev, void *cuda_stream);
 
+/* NOISE LOADING (section 6: "White noise is added to the signals before the receiver, setting the optical
+ * signal-to-noise ratio (OSNR) to 20 dB"; the reading of that sentence is R18 in DESIGN.md).  Adds complex circular white
+ * Gaussian noise, independent per row and sample, to the field in place; needs no plan and no workspace.
+ *   A_dev     device, [2M][N] complex128 in the natural layout documented at the top, 16-byte aligned; any N >= 1.
+ *   dt        sample spacing [T];  ref_bw  the OSNR's reference bandwidth [1/T] (12.5 GHz = 0.1 nm by convention);
+ *   osnr_db   requested OSNR in dB (+infinity: nothing is added);  nch >= 1  wavelength channels carried by a mode.
+ *   seed      selects the noise stream.  The sample of (seed, row, t) comes from Philox-4x32-10 with counter
+ *             (t low word, t high word, row, 0) and key (seed low word, seed high word) and Box-Muller on two 52-bit
+ *             uniforms: it does not depend on M, N or the launch, so any sub-block can be reproduced.
+ *   mode_power_dev  device, [M] doubles, OUTPUT: P_a = mean over t of |A_ax|^2 + |A_ay|^2 of the field BEFORE the noise.
+ * Per spatial mode a: noise density per polarisation N0 = P_a / (nch 2 ref_bw OSNR) (the OSNR counts the noise of both
+ * polarisations inside ref_bw against the power of one channel), white over the simulated band 1/dt, i.e. variance
+ * sigma_a^2 = N0 / dt per complex sample; A_{a,p}(t) += sigma_a z(seed, 2a+p, t) with E|z|^2 = 1.  Enqueues two kernels
+ * (mode powers: one read of the field; noise: one read and one write).  M <= 32767.
+ * mmf_debug_noise_words: the generator alone — words_dev (device, 16-byte aligned) receives the four 32-bit Philox
+ * output words of samples t0 .. t0 + count - 1 of `row`, [count][4] uint32. */
+int mmf_add_noise(void *A_dev, int M, long long N, double dt, double osnr_db, double ref_bw, int nch,
+                  unsigned long long seed, double *mode_power_dev, void *cuda_stream);
+int mmf_debug_noise_words(unsigned long long seed, unsigned row, unsigned long long t0, long long count, void *words_dev,
+                          void *cuda_stream);
+
 /* The nonlinear operator for callers that CANNOT ALLOCATE device memory: OUT <- h N(U) U of Eq. (1), as
  * mmf_apply_nonlinear computes it, but without a plan and without a workspace.
  *   Who needs it: a host program that took all of HBM for its own pool at start-up (any later cudaMalloc fails there),

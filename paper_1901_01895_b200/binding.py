@@ -21,7 +21,7 @@ SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_create_shard"
            "mmf_propagate_host", "mmf_propagate_host_batch", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
            "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_groups", "mmf_plan_set_timing", "mmf_kernel_class_count",
            "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version",
-           "mmf_probe_fp64", "mmf_probe_tma_copy", "mmf_probe_onchip", "mmf_apply_nonlinear_static"]
+           "mmf_probe_fp64", "mmf_probe_tma_copy", "mmf_probe_onchip", "mmf_apply_nonlinear_static", "mmf_add_noise", "mmf_debug_noise_words"]
 
 _lib = None
 
@@ -106,6 +106,10 @@ def lib():
     L.mmf_probe_tma_copy.restype = i
     L.mmf_apply_nonlinear_static.argtypes = [i, ll, d, d, vp, vp, vp, vp]
     L.mmf_apply_nonlinear_static.restype = i
+    L.mmf_add_noise.argtypes = [vp, i, ll, d, d, d, i, ctypes.c_ulonglong, vp, vp]
+    L.mmf_add_noise.restype = i
+    L.mmf_debug_noise_words.argtypes = [ctypes.c_ulonglong, ctypes.c_uint, ctypes.c_ulonglong, ll, vp, vp]
+    L.mmf_debug_noise_words.restype = i
     L.mmf_version.argtypes = []
     L.mmf_version.restype = ctypes.c_char_p
     _lib = L
@@ -307,6 +311,30 @@ def apply_nonlinear_static(kappa, U, OUT, h, gamma, stream=None):
                                             ctypes.c_void_p(OUT.data_ptr()), _stream_ptr(stream)),
            "mmf_apply_nonlinear_static")
     return OUT
+
+
+def add_noise(A, dt, osnr_db, ref_bw, nch, seed, mode_power=None, stream=None):
+    """mmf_add_noise: noise loading in place on the CUDA complex128 tensor A [2M][N].  Returns the CUDA
+    float64 tensor [M] of the mode powers measured before the noise (allocated here with torch unless passed in)."""
+    import torch
+    assert A.is_cuda and A.dtype == torch.complex128 and A.is_contiguous() and A.dim() == 2 and A.shape[0] % 2 == 0
+    M = A.shape[0] // 2
+    if mode_power is None:
+        mode_power = torch.empty(M, dtype=torch.float64, device=A.device)
+    assert mode_power.is_cuda and mode_power.dtype == torch.float64 and mode_power.numel() == M
+    _check(lib().mmf_add_noise(ctypes.c_void_p(A.data_ptr()), int(M), int(A.shape[1]), float(dt), float(osnr_db),
+                               float(ref_bw), int(nch), int(seed), ctypes.c_void_p(mode_power.data_ptr()),
+                               _stream_ptr(stream)), "mmf_add_noise")
+    return mode_power
+
+
+def noise_words(seed, row, t0, count, device="cuda:0", stream=None):
+    """mmf_debug_noise_words: CUDA int32 tensor [count][4] holding the Philox output words (as uint32 bit patterns)."""
+    import torch
+    out = torch.empty((int(count), 4), dtype=torch.int32, device=device)
+    _check(lib().mmf_debug_noise_words(int(seed), int(row), int(t0), int(count), ctypes.c_void_p(out.data_ptr()),
+                                       _stream_ptr(stream)), "mmf_debug_noise_words")
+    return out
 
 
 def raw_create(M, N, dt, h, alpha, beta, K, gamma, kappa, general=False):

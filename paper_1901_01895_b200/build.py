@@ -1,14 +1,22 @@
-"""Build libmmf_b200.so (the C-ABI CUDA library of include/mmf.h) in-tree with nvcc for sm_100a."""
+"""Build libmmf_b200.so (the C-ABI CUDA library of include/mmf.h) in-tree with nvcc for sm_100a.
+
+Every translation unit is compiled to an object of its own (kept under paper_1901_01895_b200/build/, git-ignored) and
+recompiled only when it or one of the files it includes is newer; the objects are then linked into the one library."""
 import os
 import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmmf_b200.so")
-SOURCES = [os.path.join(CSRC, "mmf_api.cu"), os.path.join(CSRC, "probes.cu"), os.path.join(CSRC, "nl_static.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fft_core.cuh", "fft_kernels.cuh", "nl_tma.cuh", "async_copy.cuh", "nl_simt.cuh", "nl_general.cuh", "nl_shard.cuh", "small_cluster.cuh", "tmem_exchange.cuh", "probes.cu")] + [
-    os.path.join(os.path.dirname(HERE), "include", "mmf.h")]
+HEADER = os.path.join(os.path.dirname(HERE), "include", "mmf.h")
+CUH = [os.path.join(CSRC, f) for f in ("fft_core.cuh", "fft_kernels.cuh", "nl_tma.cuh", "async_copy.cuh", "nl_simt.cuh",
+                                       "nl_general.cuh", "nl_shard.cuh", "small_cluster.cuh", "tmem_exchange.cuh")]
+# translation unit -> the files it includes (besides itself)
+UNITS = {"mmf_api.cu": CUH + [HEADER], "probes.cu": CUH + [HEADER], "nl_static.cu": [HEADER], "noise.cu": [HEADER]}
+SOURCES = [os.path.join(CSRC, u) for u in UNITS]
+FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
 def nvcc_path():
@@ -18,17 +26,29 @@ def nvcc_path():
     return "nvcc"
 
 
+def _stale(target, deps):
+    return not os.path.exists(target) or any(os.path.getmtime(target) < os.path.getmtime(d) for d in deps)
+
+
 def build(force=False, verbose=False):
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
-        return LIB
-    tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-           "-Xcompiler", "-fPIC", "-shared", "-o", tmp] + SOURCES
-    if verbose:
-        cmd.insert(1, "-Xptxas")
-        cmd.insert(2, "-v")
-    subprocess.run(cmd, check=True)
-    os.replace(tmp, LIB)
+    me = os.path.abspath(__file__)
+    os.makedirs(OBJ, exist_ok=True)
+    objs, procs = [], []
+    for unit, deps in UNITS.items():
+        src = os.path.join(CSRC, unit)
+        obj = os.path.join(OBJ, unit.replace(".cu", ".o"))
+        objs.append(obj)
+        if force or _stale(obj, [src, me] + deps):
+            cmd = [nvcc_path()] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj + ".tmp"]
+            procs.append((obj, cmd, subprocess.Popen(cmd)))      # the units compile side by side
+    for obj, cmd, pr in procs:
+        if pr.wait() != 0:
+            raise subprocess.CalledProcessError(pr.returncode, cmd)
+        os.replace(obj + ".tmp", obj)
+    if procs or _stale(LIB, objs):
+        tmp = LIB + ".tmp.%d" % os.getpid()
+        subprocess.run([nvcc_path(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs, check=True)
+        os.replace(tmp, LIB)
     return LIB
 
 
