@@ -272,3 +272,32 @@ def test_full_length_matches_golden(mmf, torch, cfg):
     assert err_d.max() <= TOL_FIELD, (err_d.max(), err_d.argmax())
     assert err_a.max() <= TOL_FIELD, (err_a.max(), err_a.argmax())
     assert np.abs(norm2 / g["norm2"] - 1.0).max() <= 1e-10
+
+
+def test_cfg4_own_seeded_field_two_steps_matches_golden(mmf, torch):
+    """Config 4 (M = 120, N = 2^22) on ITS OWN seeded, non-periodic field (every bin inside the band occupied), the
+    plan bench.py times, 2 whole RK4IP steps: sampled against the oracle's stored output (tests/golden/make_golden.py
+    4:2, run once on the GPU box's host cores), plus the energy of every row.  The 50-step test above covers the step
+    count on a periodic tiling; this one covers the real field."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg4_2steps.npz")
+    g = np.load(path)
+    p = workloads.problem(4)
+    cfg, M, N, steps = (int(x) for x in g["meta"])
+    assert (cfg, M, N) == (4, p.M, p.N) and steps == 2
+    A = field_threaded(p)
+    pl = plan_for(mmf, p)
+    X = torch.from_numpy(A).to("cuda:0")
+    del A
+    pl.propagate(X, steps)
+    torch.cuda.synchronize()
+    dev = X.device
+    rows, idx_d, idx_a = (torch.from_numpy(g[k]).to(dev) for k in ("rows_dense", "idx_dense", "idx_all"))
+    got_d = X[rows][:, idx_d].cpu().numpy()
+    got_a = X[:, idx_a].cpu().numpy()
+    norm2 = np.array([float((X[r].real ** 2 + X[r].imag ** 2).sum()) for r in range(X.shape[0])])
+    err_d = workloads.rel_l2_per_field(got_d, g["dense"])
+    err_a = workloads.rel_l2_per_field(got_a, g["all"])
+    assert err_d.max() <= TOL_FIELD, (err_d.max(), err_d.argmax())
+    assert err_a.max() <= TOL_FIELD, (err_a.max(), err_a.argmax())
+    assert np.abs(norm2 / g["norm2"] - 1.0).max() <= 1e-10
+    pl.destroy()
