@@ -21,9 +21,14 @@ SYMBOLS = ["mmf_plan_create", "mmf_plan_create_general", "mmf_plan_create_shard"
            "mmf_propagate_host", "mmf_propagate_host_batch", "mmf_apply_linear", "mmf_apply_nonlinear", "mmf_debug_forward",
            "mmf_debug_freq_index", "mmf_plan_launch_count", "mmf_plan_groups", "mmf_plan_set_timing", "mmf_kernel_class_count",
            "mmf_kernel_class_name", "mmf_plan_get_timing", "mmf_plan_destroy", "mmf_status_string", "mmf_version",
-           "mmf_probe_fp64", "mmf_probe_tma_copy", "mmf_probe_onchip", "mmf_apply_nonlinear_static", "mmf_add_noise", "mmf_debug_noise_words"]
+           "mmf_apply_nonlinear_static", "mmf_add_noise", "mmf_debug_noise_words"]
+
+# every symbol include/mmf_probes.h declares (libmmf_probes.so: measurement probes, not part of the product library)
+PROBE_SYMBOLS = ["mmf_probe_fp64", "mmf_probe_tma_copy", "mmf_probe_onchip"]
+PROBES_LIB_PATH = os.path.join(_HERE, "libmmf_probes.so")
 
 _lib = None
+_probes = None
 
 
 class MmfError(RuntimeError):
@@ -97,13 +102,6 @@ def lib():
     L.mmf_plan_destroy.restype = i
     L.mmf_status_string.argtypes = [i]
     L.mmf_status_string.restype = ctypes.c_char_p
-    ull, u = ctypes.c_ulonglong, ctypes.c_uint
-    L.mmf_probe_fp64.argtypes = [i, i, i, dp, dp]
-    L.mmf_probe_fp64.restype = i
-    L.mmf_probe_onchip.argtypes = [i, i, i, dp, dp]
-    L.mmf_probe_onchip.restype = i
-    L.mmf_probe_tma_copy.argtypes = [vp, sz, ull, ull, ull, u, u, i, i, i, i, ll, i, i, i, dp, dp]
-    L.mmf_probe_tma_copy.restype = i
     L.mmf_apply_nonlinear_static.argtypes = [i, ll, d, d, vp, vp, vp, vp]
     L.mmf_apply_nonlinear_static.restype = i
     L.mmf_add_noise.argtypes = [vp, i, ll, d, d, d, i, ctypes.c_ulonglong, vp, vp]
@@ -113,6 +111,27 @@ def lib():
     L.mmf_version.argtypes = []
     L.mmf_version.restype = ctypes.c_char_p
     _lib = L
+    return L
+
+
+def probes_lib():
+    """Load libmmf_probes.so (bench.py --probes).  Fails loudly if absent."""
+    global _probes
+    if _probes is not None:
+        return _probes
+    if not os.path.exists(PROBES_LIB_PATH):
+        raise MmfError("probe library %s is missing: run `python -m paper_1901_01895_b200.build`" % PROBES_LIB_PATH)
+    L = ctypes.CDLL(PROBES_LIB_PATH)
+    i, d, sz, vp, ll = ctypes.c_int, ctypes.c_double, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_longlong
+    dp = ctypes.POINTER(ctypes.c_double)
+    ull, u = ctypes.c_ulonglong, ctypes.c_uint
+    L.mmf_probe_fp64.argtypes = [i, i, i, dp, dp]
+    L.mmf_probe_fp64.restype = i
+    L.mmf_probe_onchip.argtypes = [i, i, i, dp, dp]
+    L.mmf_probe_onchip.restype = i
+    L.mmf_probe_tma_copy.argtypes = [vp, sz, ull, ull, ull, u, u, i, i, i, i, ll, i, i, i, dp, dp]
+    L.mmf_probe_tma_copy.restype = i
+    _probes = L
     return L
 
 
@@ -351,14 +370,14 @@ def raw_create(M, N, dt, h, alpha, beta, K, gamma, kappa, general=False):
 def probe_fp64(kind, threads=512, iters=4000):
     """mmf_probe_fp64: (ms per launch, thread-level (kind 5: warp-level) instructions per launch)."""
     ms, n = ctypes.c_double(), ctypes.c_double()
-    _check(lib().mmf_probe_fp64(int(kind), int(threads), int(iters), ctypes.byref(ms), ctypes.byref(n)), "mmf_probe_fp64")
+    _check(probes_lib().mmf_probe_fp64(int(kind), int(threads), int(iters), ctypes.byref(ms), ctypes.byref(n)), "mmf_probe_fp64")
     return ms.value, n.value
 
 
 def probe_onchip(kind, threads=512, iters=2000):
     """mmf_probe_onchip: (ms per launch, clock64 ticks per operation with every warp of the CTA running the loop)."""
     ms, clk = ctypes.c_double(), ctypes.c_double()
-    _check(lib().mmf_probe_onchip(int(kind), int(threads), int(iters), ctypes.byref(ms), ctypes.byref(clk)),
+    _check(probes_lib().mmf_probe_onchip(int(kind), int(threads), int(iters), ctypes.byref(ms), ctypes.byref(clk)),
            "mmf_probe_onchip")
     return ms.value, clk.value
 
@@ -367,7 +386,7 @@ def probe_tma_copy(buf, dim0, dim1, stride_bytes, box0, box1, nbox, nct_log, c0_
                    reps=3):
     """mmf_probe_tma_copy over the torch uint8 CUDA tensor `buf`: (ms per launch, bytes moved read + write)."""
     ms, by = ctypes.c_double(), ctypes.c_double()
-    _check(lib().mmf_probe_tma_copy(ctypes.c_void_p(buf.data_ptr()), buf.numel(), int(dim0), int(dim1), int(stride_bytes),
+    _check(probes_lib().mmf_probe_tma_copy(ctypes.c_void_p(buf.data_ptr()), buf.numel(), int(dim0), int(dim1), int(stride_bytes),
                                     int(box0), int(box1), int(nbox), int(nct_log), int(c0_mul), int(c1_mul), int(ntiles),
                                     int(slots), int(bulk), int(reps), ctypes.byref(ms), ctypes.byref(by)),
            "mmf_probe_tma_copy")

@@ -132,7 +132,7 @@ struct mmf_plan {
   size_t ws_bytes = 0, field_bytes = 0;
   cpx *Y = nullptr, *Z = nullptr, *W = nullptr, *V = nullptr, *E = nullptr;
   double* T = nullptr;  // N <= 4096: the table of mmf_propagate_ssfm_agrawal (workspace)
-  // launch plan: everything a launch needs besides its arguments is computed once per plan —
+  // launch plan ("small-problem launch plan"): everything a launch needs besides its arguments is computed once per plan —
   // tensor maps per (kind, buffer), the dynamic shared-memory attribute and the occupancy per kernel — and the step
   // body of small problems is replayed from a captured CUDA graph
   struct MapEntry { int kind; const void* base; int aux; CUtensorMap map; };

@@ -5,7 +5,7 @@
 #include <cstdio>
 #include <cstring>
 
-#include "../../include/mmf.h"
+#include "../../include/mmf_probes.h"
 #include "async_copy.cuh"
 #include "tmem_exchange.cuh"
 

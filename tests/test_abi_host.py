@@ -23,6 +23,12 @@ def test_library_exports_every_declared_symbol(mmf):
     L = mmf.lib()
     for s in declared:
         assert hasattr(L, s), s
+    ph = open(os.path.join(ROOT, "include", "mmf_probes.h")).read()
+    probes = set(re.findall(r"\b(mmf_[a-z0-9_]+)\s*\(", ph))
+    assert probes == set(mmf.PROBE_SYMBOLS), probes ^ set(mmf.PROBE_SYMBOLS)
+    PL = mmf.probes_lib()
+    for s in probes:
+        assert hasattr(PL, s) and not hasattr(L, s), s       # the product library carries the product only
     assert L.mmf_version().startswith(b"mmf-b200")
     assert L.mmf_status_string(mmf.MMF_EINVAL) == b"invalid argument"
 
